@@ -1,0 +1,170 @@
+/*
+ * g3.h -- C ABI of libg3: the triplet correlation function g(3) of a particle
+ * trajectory on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arxiv 1708.08619 section 3.2.  g(3) is defined by Eq. 3
+ * (PAPER.md:403-405); it is computed as a "3D histogram binning of distances
+ * with imposed conditions": for every central particle i
+ * and every pair (j,k) of its neighbours inside the cut-off, the three pair
+ * distances (r_ij, r_ik, r_jk) select one bin.  Algorithm 6
+ * is the serial form, Algorithm 7 the GPU form the paper
+ * used: CUDA_g2 stores each particle's minimum-image neighbour vectors,
+ * CUDA_g3 bins the j-k distance computed from those stored vectors.  Where
+ * the paper is silent, DESIGN.md ("Readings of the paper") fixes the reading.
+ *
+ * Exact definition implemented:
+ *   grid      positions are snapped to the box/2^20 grid:
+ *             m = llrint(x * (2^20/box)) mod 2^20 per coordinate;
+ *   edges     T_r[b] = ceil((b*w)^2), w = (r_max/n_r)*(2^20/box), b = 0..n_r
+ *             T_t[c] = ceil((c*wt)^2), wt = ((2*r_max)/n_t)*(2^20/box), c = 0..n_t
+ *             (fp64, one rounding per operation); bin(T,q) = max{b : T[b] <= q};
+ *   neighbour j != i with minimum-image vector d_j (components in [-2^19, 2^19))
+ *             and |d_j|^2 < T_r[n_r]; shell a_j = bin(T_r, |d_j|^2);
+ *   triplet   every ORDERED pair (j,k), j != k, of neighbours of i:
+ *             t2 = |d_k - d_j|^2 (no second minimum image), c = bin(T_t, t2);
+ *             c < n_t  ->  counts[a_j][a_k][c] += 1, else overflow += 1;
+ *   g3        counts / (frames * n * rho^2 * V_abc), rho = n/box^3, V_abc the
+ *             integral of 8 pi^2 r s t over the part of the bin that obeys
+ *             |r-s| <= t <= r+s; 0 where V_abc = 0.
+ * counts is symmetric in its first two axes; the number of DISTINCT triplets is
+ * (sum(counts) + overflow) / 2 = sum_i C(k_i, 2).
+ *
+ * General rules
+ *   - Every function returns a g3_status (int); nothing throws, aborts or prints.
+ *   - "device" pointers are CUDA device pointers on the plan's GPU; "host"
+ *     pointers are ordinary host memory.  `stream` is a cudaStream_t passed as
+ *     void* (NULL = the legacy default stream).
+ *   - The plan owns all scratch memory and the running histogram.  The caller
+ *     owns every buffer it passes in.
+ *   - A plan is not thread-safe; distinct plans are independent.  All calls on
+ *     one plan must be issued on one stream, or be ordered by the caller.
+ *   - The library never falls back to the CPU: if no CUDA device is usable,
+ *     g3_plan_create fails with G3_ECUDA.
+ */
+#ifndef G3_H_
+#define G3_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define G3_API __attribute__((visibility("default")))
+#else
+#define G3_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct g3_plan g3_plan; /* opaque; created by g3_plan_create, freed by g3_plan_destroy */
+
+/* Bin specification.  r_ij and r_ik: n_r uniform bins on [0, r_max).
+ * r_jk: n_t uniform bins on [0, 2*r_max).  1 <= n_r, n_t <= 1024. */
+typedef struct {
+    int32_t n_r;
+    int32_t n_t;
+} g3_bins;
+
+typedef enum {
+    G3_OK = 0,
+    G3_EINVAL = 1,    /* bad argument (see each function)                                   */
+    G3_ENOMEM = 2,    /* host or device allocation failed                                   */
+    G3_ECUDA = 3,     /* a CUDA runtime call failed, or no sm_100 device is present         */
+    G3_ECAPACITY = 4, /* a central particle had more neighbours than the plan can hold      */
+    G3_ESTATE = 5     /* call not valid in the plan's current state                         */
+} g3_status;
+
+/* Options for g3_plan_set_option (all optional; defaults are chosen for the B200). */
+typedef enum {
+    G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1)      */
+    G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
+    G3_OPT_MAX_NEIGHBOURS = 3 /* per-centre neighbour capacity (0 = derive from density)     */
+} g3_option;
+
+/* Keys for g3_plan_get_info. */
+typedef enum {
+    G3_INFO_KERNEL_LAUNCHES = 1, /* kernels launched by this plan since creation / reset     */
+    G3_INFO_BATCH_FRAMES = 2,
+    G3_INFO_KERNEL = 3,          /* kernel actually selected (1 or 2)                        */
+    G3_INFO_CELLS_PER_EDGE = 4,
+    G3_INFO_MAX_NEIGHBOURS = 5,
+    G3_INFO_TILE_BINS = 6,       /* histogram bins privatised in shared memory per CTA       */
+    G3_INFO_SM_COUNT = 7,
+    G3_INFO_FRAMES_PENDING = 8   /* staged frames not yet reduced into the histogram         */
+} g3_info;
+
+/* Create a plan for frames of `n` particles in a cubic periodic box of edge `box`
+ * (positions + box lengths; cubic because the paper's cut-offs
+ * are fractions of one "Boxlength").
+ *   n      >= 3
+ *   box    > 0, same length unit as the positions
+ *   r_max  cut-off on r_ij and r_ik (replaces the paper's Boxlength/4,
+ *          PAPER.md:407); 0 < r_max < box/2 so that the minimum image is unique
+ *   bins   see g3_bins
+ * On success *out holds the plan and its histogram is zero.  Uses the CUDA device
+ * current at the time of the call for the whole life of the plan.
+ * Errors: G3_EINVAL (null out, bad n/box/r_max/bins), G3_ENOMEM, G3_ECUDA.          */
+G3_API int g3_plan_create(g3_plan **out, int64_t n, double box, double r_max, g3_bins bins);
+
+/* Tune a plan before the first frame.  G3_ESTATE after frames were accumulated
+ * (until g3_plan_reset), G3_EINVAL for unknown keys or bad values.                  */
+G3_API int g3_plan_set_option(g3_plan *p, int32_t option, int64_t value);
+G3_API int g3_plan_get_info(const g3_plan *p, int32_t key, int64_t *value);
+
+/* Add one frame (Algorithm 6/7's loop body).
+ *   d_pos  device, fp64, [n][3] row-major (x,y,z of particle 0, then particle 1, ...).
+ *          Any real coordinate is accepted: it is snapped to the box/2^20 grid and
+ *          wrapped into the box.
+ * Asynchronous and stream-ordered: never synchronises the host.  d_pos is fully
+ * consumed by work enqueued during this call (it is quantised into plan-owned
+ * staging), so it may be reused as soon as `stream` has passed this call.  The
+ * triplet work itself may be deferred until G3_OPT_BATCH_FRAMES frames are staged
+ * or g3_finalize is called; results are identical either way.
+ * Errors: G3_EINVAL (null), G3_ECUDA.                                               */
+G3_API int g3_accumulate_frame(g3_plan *p, const double *d_pos, void *stream);
+
+/* Same as calling g3_accumulate_frame for f = 0..n_frames-1 on d_pos + f*frame_stride
+ * (frame_stride in doubles, >= 3*n), with one batched launch sequence.              */
+G3_API int g3_accumulate_frames(g3_plan *p, const double *d_pos, int64_t n_frames, int64_t frame_stride,
+                         void *stream);
+
+/* Same, from HOST memory (pinned memory gives asynchronous copies; pageable works).
+ * Copies are issued on `stream` in chunks that overlap with compute.  h_pos must
+ * stay valid until `stream` has passed this call.                                   */
+G3_API int g3_accumulate_frames_host(g3_plan *p, const double *h_pos, int64_t n_frames,
+                              int64_t frame_stride, void *stream);
+
+/* Reduce all staged frames, then write the results and SYNCHRONISE `stream`.
+ *   d_counts  device, uint64 [n_r][n_r][n_t], c (r_jk bin) fastest; may be NULL
+ *   d_g3      device, fp64, same shape: counts / (frames n rho^2 V_abc); may be NULL
+ *   h_stats   host, uint64[3] = { frames, sum_i k_i (k_i - 1), overflow }; may be NULL
+ * Does not reset the plan: more frames may follow, and it may be called again.
+ * Errors: G3_ECAPACITY if any centre exceeded the neighbour capacity (counts are
+ * then incomplete), G3_ECUDA.                                                       */
+G3_API int g3_finalize(g3_plan *p, uint64_t *d_counts, double *d_g3, uint64_t *h_stats, void *stream);
+
+/* Same with HOST output buffers (device-to-host copies included).                   */
+G3_API int g3_finalize_host(g3_plan *p, uint64_t *h_counts, double *h_g3, uint64_t *h_stats, void *stream);
+
+/* Normalise externally merged counts (e.g. the sum over ranks of a frame-sharded
+ * run; the paper's "split the trajectory, merge the results"):
+ * d_g3 = d_counts / (frames n rho^2 V_abc).  Asynchronous on `stream`.              */
+G3_API int g3_normalize(g3_plan *p, const uint64_t *d_counts, uint64_t frames, double *d_g3, void *stream);
+
+/* Copy the plan's bin-volume table V_abc (fp64 [n_r][n_r][n_t], units of box^6
+ * length) to host memory.                                                           */
+G3_API int g3_bin_volumes(const g3_plan *p, double *h_volumes);
+
+/* Zero the histogram, frame count and error state; keep all buffers.                */
+G3_API int g3_plan_reset(g3_plan *p, void *stream);
+
+/* Free the plan (NULL is allowed).  Synchronises the device.                        */
+G3_API void g3_plan_destroy(g3_plan *p);
+
+/* Static description of a status code.                                              */
+G3_API const char *g3_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* G3_H_ */

@@ -1,0 +1,200 @@
+"""Thin ctypes binding of libg3 (include/g3.h).  Argument marshalling only: every step of the
+g(3) path runs in the CUDA kernels behind the C ABI.  torch supplies device memory and streams.
+
+There is no CPU fallback: importing works anywhere (so the ABI can be inspected), but creating a
+plan without the built library or without a B200 raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libg3.so")
+
+G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
+G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS = 1, 2, 3
+(G3_INFO_KERNEL_LAUNCHES, G3_INFO_BATCH_FRAMES, G3_INFO_KERNEL, G3_INFO_CELLS_PER_EDGE,
+ G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING) = range(1, 9)
+
+EXPORTS = [
+    "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_accumulate_frame",
+    "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
+    "g3_normalize", "g3_bin_volumes", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+]
+
+
+class g3_bins(C.Structure):
+    _fields_ = [("n_r", C.c_int32), ("n_t", C.c_int32)]
+
+
+class G3Error(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {strerror(code)} (g3_status {code})")
+        self.code = code
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def load() -> C.CDLL:
+    """dlopen libg3.so (built by paper_1708_08619_b200.build).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1708_08619_b200.build` "
+                           "(needs nvcc). There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, i32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+    lib.g3_plan_create.argtypes = [C.POINTER(vp), i64, f64, f64, g3_bins]
+    lib.g3_plan_set_option.argtypes = [vp, i32, i64]
+    lib.g3_plan_get_info.argtypes = [vp, i32, C.POINTER(i64)]
+    lib.g3_accumulate_frame.argtypes = [vp, vp, vp]
+    lib.g3_accumulate_frames.argtypes = [vp, vp, i64, i64, vp]
+    lib.g3_accumulate_frames_host.argtypes = [vp, vp, i64, i64, vp]
+    lib.g3_finalize.argtypes = [vp, vp, vp, vp, vp]
+    lib.g3_finalize_host.argtypes = [vp, vp, vp, vp, vp]
+    lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
+    lib.g3_bin_volumes.argtypes = [vp, vp]
+    lib.g3_plan_reset.argtypes = [vp, vp]
+    lib.g3_plan_destroy.argtypes = [vp]
+    lib.g3_plan_destroy.restype = None
+    lib.g3_strerror.argtypes = [C.c_int]
+    lib.g3_strerror.restype = C.c_char_p
+    for name in EXPORTS:
+        if name not in ("g3_plan_destroy", "g3_strerror"):
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load().g3_strerror(int(code)).decode()
+
+
+def _check(code: int, what: str, allow=()):
+    if code != G3_OK and code not in allow:
+        raise G3Error(code, what)
+    return code
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Plan:
+    """g3_plan with the same calls as the C ABI: accumulate_frame(s), finalize, reset."""
+
+    def __init__(self, n: int, box: float, r_max: float, n_r: int, n_t: Optional[int] = None, *,
+                 batch_frames: Optional[int] = None, kernel: Optional[int] = None,
+                 max_neighbours: Optional[int] = None):
+        self._lib = load()
+        self.n, self.box, self.r_max = int(n), float(box), float(r_max)
+        self.n_r, self.n_t = int(n_r), int(n_r if n_t is None else n_t)
+        self._h = C.c_void_p()
+        _check(self._lib.g3_plan_create(C.byref(self._h), self.n, self.box, self.r_max,
+                                        g3_bins(self.n_r, self.n_t)), "g3_plan_create")
+        if batch_frames is not None:
+            self.set_option(G3_OPT_BATCH_FRAMES, batch_frames)
+        if kernel is not None:
+            self.set_option(G3_OPT_KERNEL, kernel)
+        if max_neighbours is not None:
+            self.set_option(G3_OPT_MAX_NEIGHBOURS, max_neighbours)
+
+    # -- options / info -------------------------------------------------------------------
+    def set_option(self, option: int, value: int) -> None:
+        _check(self._lib.g3_plan_set_option(self._h, option, int(value)), "g3_plan_set_option")
+
+    def info(self, key: int) -> int:
+        v = C.c_int64()
+        _check(self._lib.g3_plan_get_info(self._h, key, C.byref(v)), "g3_plan_get_info")
+        return int(v.value)
+
+    @property
+    def shape(self) -> Tuple[int, int, int]:
+        return (self.n_r, self.n_r, self.n_t)
+
+    # -- accumulation ---------------------------------------------------------------------
+    def _check_pos(self, pos, device_type: str, frames: bool):
+        import torch
+        if pos.dtype != torch.float64 or pos.device.type != device_type or not pos.is_contiguous():
+            raise ValueError(f"positions must be a contiguous float64 {device_type} tensor")
+        want = (self.n, 3)
+        if tuple(pos.shape[-2:]) != want or pos.dim() != (3 if frames else 2):
+            raise ValueError(f"positions must have shape {'[F,' if frames else '['}{self.n},3]")
+
+    def accumulate_frame(self, d_pos, stream=None) -> None:
+        self._check_pos(d_pos, "cuda", False)
+        _check(self._lib.g3_accumulate_frame(self._h, d_pos.data_ptr(), _stream_ptr(stream)),
+               "g3_accumulate_frame")
+
+    def accumulate_frames(self, d_pos, stream=None) -> None:
+        self._check_pos(d_pos, "cuda", True)
+        _check(self._lib.g3_accumulate_frames(self._h, d_pos.data_ptr(), d_pos.shape[0], 3 * self.n,
+                                              _stream_ptr(stream)), "g3_accumulate_frames")
+
+    def accumulate_frames_host(self, h_pos, stream=None) -> None:
+        self._check_pos(h_pos, "cpu", True)
+        _check(self._lib.g3_accumulate_frames_host(self._h, h_pos.data_ptr(), h_pos.shape[0],
+                                                   3 * self.n, _stream_ptr(stream)),
+               "g3_accumulate_frames_host")
+
+    # -- results --------------------------------------------------------------------------
+    def finalize(self, want_g3: bool = True, stream=None):
+        """(counts int64-viewed-as-uint64 device tensor, g3 device tensor or None, stats list)."""
+        import torch
+        counts = torch.empty(self.shape, dtype=torch.int64, device="cuda")   # bit pattern of uint64
+        g3 = torch.empty(self.shape, dtype=torch.float64, device="cuda") if want_g3 else None
+        stats = (C.c_uint64 * 3)()
+        _check(self._lib.g3_finalize(self._h, counts.data_ptr(), g3.data_ptr() if want_g3 else None,
+                                     stats, _stream_ptr(stream)), "g3_finalize")
+        return counts, g3, [int(v) for v in stats]
+
+    def finalize_host(self, want_g3: bool = True, stream=None):
+        import torch
+        counts = torch.empty(self.shape, dtype=torch.int64).pin_memory()
+        g3 = torch.empty(self.shape, dtype=torch.float64).pin_memory() if want_g3 else None
+        stats = (C.c_uint64 * 3)()
+        _check(self._lib.g3_finalize_host(self._h, counts.data_ptr(), g3.data_ptr() if want_g3 else None,
+                                          stats, _stream_ptr(stream)), "g3_finalize_host")
+        return counts, g3, [int(v) for v in stats]
+
+    def normalize(self, d_counts, frames: int, stream=None):
+        import torch
+        if d_counts.dtype != torch.int64 or d_counts.device.type != "cuda" or not d_counts.is_contiguous():
+            raise ValueError("counts must be a contiguous int64 cuda tensor")
+        g3 = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        _check(self._lib.g3_normalize(self._h, d_counts.data_ptr(), int(frames), g3.data_ptr(),
+                                      _stream_ptr(stream)), "g3_normalize")
+        return g3
+
+    def bin_volumes(self):
+        import numpy as np
+        V = np.empty(self.shape, dtype=np.float64)
+        _check(self._lib.g3_bin_volumes(self._h, V.ctypes.data_as(C.c_void_p)), "g3_bin_volumes")
+        return V
+
+    def reset(self, stream=None) -> None:
+        _check(self._lib.g3_plan_reset(self._h, _stream_ptr(stream)), "g3_plan_reset")
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.g3_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,82 @@
+// g3_plan.h -- internal plan state of libg3 (not part of the public ABI, see include/g3.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/g3.h"
+
+namespace g3 {
+
+constexpr int kGridBits = 20;                 // positions live on the box/2^20 grid
+constexpr int64_t kGrid = int64_t(1) << kGridBits;
+constexpr int kMaxCellsPerEdge = 32;          // cell ids fit 15 bits
+
+// Device-visible description of one batch of staged frames.  Passed by value to kernels.
+struct FrameBatch {
+    int32_t n;                 // particles per frame
+    int32_t n_frames;          // frames in this batch
+    int32_t ncell;             // cells per edge (1 = no cell grid: every particle is a candidate)
+    int32_t ncell3;
+    const int4* sorted;        // [frames][n]  (x, y, z, cell id), cell-major order
+    const int32_t* cell_start; // [frames][ncell3 + 1]
+};
+
+struct BinSpec {
+    int32_t n_r, n_t;
+    const unsigned long long* T_r;  // device, [n_r + 1] squared edges in grid units
+    const unsigned long long* T_t;  // device, [n_t + 1]
+    unsigned long long cut2;        // T_r[n_r]
+};
+
+}  // namespace g3
+
+struct g3_plan {
+    // problem
+    int64_t n = 0;
+    double box = 0, r_max = 0;
+    g3_bins bins{0, 0};
+    int64_t nbins = 0;
+    double inv_g = 0;                        // 2^20 / box
+    std::vector<unsigned long long> T_r, T_t; // host copies of the squared edges
+    std::vector<double> volumes;             // V_abc in box length units^6 (host)
+
+    // device
+    int device = -1;
+    int sm_count = 0;
+    int smem_optin = 0;
+
+    // options / derived
+    int32_t batch_frames = 16;
+    int32_t kernel_opt = 0;                  // G3_OPT_KERNEL
+    int32_t kernel = 1;                      // selected kernel
+    int32_t ncell = 1;
+    int32_t max_nb = 0;                      // neighbour capacity per centre
+    int32_t max_nb_opt = 0;
+    int64_t tile_bins = 0;
+
+    // device buffers
+    unsigned long long* d_T_r = nullptr;
+    unsigned long long* d_T_t = nullptr;
+    unsigned long long* d_counts = nullptr;  // [nbins] running histogram (ordered pairs)
+    unsigned long long* d_stats = nullptr;   // [4]: pairs, overflow, capacity error, spare
+    double* d_volumes = nullptr;             // [nbins]
+    int4* d_staged = nullptr;                // [batch][n] quantised (x,y,z,cell) in input order
+    int32_t* d_slot = nullptr;               // [batch][n] rank of the particle inside its cell
+    int32_t* d_cell_count = nullptr;         // [batch][ncell3]
+    int32_t* d_cell_start = nullptr;         // [batch][ncell3 + 1]
+    int4* d_sorted = nullptr;                // [batch][n]
+    double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
+    cudaEvent_t h2d_done[2] = {nullptr, nullptr};
+    int64_t h2d_chunk_frames = 0;
+    void* d_tiled_scratch = nullptr;         // owned by the tiled kernel (work counters etc.)
+    size_t tiled_scratch_bytes = 0;
+
+    // state
+    int32_t pending = 0;                     // frames staged, not yet reduced
+    uint64_t frames = 0;                     // frames accumulated in total (staged included)
+    uint64_t launches = 0;                   // kernels launched
+    bool configured = false;                 // buffers allocated for the current options
+};

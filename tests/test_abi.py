@@ -1,0 +1,73 @@
+"""CPU-side checks of the boundary: libg3.so builds for sm_100a, loads, and exports every
+symbol include/g3.h declares.  No compute calls (no GPU here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1708_08619_b200 import build
+    build.build()
+    import paper_1708_08619_b200 as g3
+    return g3.load()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "g3.h")).read()
+    return re.findall(r"G3_API\s+[\w\s\*]+?\b(g3_\w+)\s*\(", text)
+
+
+def test_header_symbols_exported(lib):
+    names = declared_symbols()
+    assert len(names) >= 10 and "g3_plan_create" in names and "g3_finalize" in names
+    for name in names:
+        assert hasattr(lib, name), name
+
+
+def test_binding_lists_the_same_names(lib):
+    import paper_1708_08619_b200 as g3
+    assert sorted(g3.EXPORTS) == sorted(declared_symbols())
+
+
+def test_strerror_and_argument_errors(lib):
+    import paper_1708_08619_b200 as g3
+    assert g3.strerror(g3.G3_OK) == "ok"
+    assert "capacity" in g3.strerror(g3.G3_ECAPACITY)
+    h = ctypes.c_void_p()
+    bins = g3.binding.g3_bins(8, 8)
+    # argument validation happens before any CUDA call
+    assert lib.g3_plan_create(None, 100, 1.0, 0.2, bins) == g3.G3_EINVAL
+    assert lib.g3_plan_create(ctypes.byref(h), 2, 1.0, 0.2, bins) == g3.G3_EINVAL        # n < 3
+    assert lib.g3_plan_create(ctypes.byref(h), 100, 1.0, 0.5, bins) == g3.G3_EINVAL      # r_max >= box/2
+    assert lib.g3_plan_create(ctypes.byref(h), 100, -1.0, 0.2, bins) == g3.G3_EINVAL
+    assert lib.g3_plan_create(ctypes.byref(h), 100, 1.0, 0.2, g3.binding.g3_bins(0, 8)) == g3.G3_EINVAL
+    assert h.value is None
+    assert lib.g3_accumulate_frame(None, None, None) == g3.G3_EINVAL
+    assert lib.g3_finalize(None, None, None, None, None) == g3.G3_EINVAL
+    lib.g3_plan_destroy(None)
+
+
+def test_no_cpu_fallback_without_gpu(lib):
+    """On a box without a CUDA device plan creation must fail loudly, never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import paper_1708_08619_b200 as g3
+    with pytest.raises(g3.G3Error) as e:
+        g3.Plan(100, 1.0, 0.2, 8)
+    assert e.value.code == g3.G3_ECUDA
+
+
+def test_product_does_not_touch_oracle():
+    """The product package must not import, read or link anything under oracle/."""
+    pkg = os.path.join(ROOT, "paper_1708_08619_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert "oracle" not in text.lower(), os.path.join(dirpath, fn)

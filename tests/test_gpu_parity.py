@@ -1,0 +1,186 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle: uint64 counts and the
+overflow/pair statistics bit-exact, g3 to relative 1e-12 (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+from workloads import GRID, WORKLOADS, frames, grid_to_pos, uniform_frame
+
+pytestmark = pytest.mark.gpu
+
+G3_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def g3():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1708_08619_b200 import build
+    build.build()
+    import paper_1708_08619_b200 as g3
+    g3.load()
+    return g3
+
+
+def run_gpu(g3, pos, box, r_max, n_r, n_t, **opts):
+    import torch
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    if pos.ndim == 2:
+        pos = pos[None]
+    with g3.Plan(pos.shape[1], box, r_max, n_r, n_t, **opts) as plan:
+        d = torch.from_numpy(pos).cuda()
+        plan.accumulate_frames(d)
+        counts, g3v, stats = plan.finalize()
+        info = {"kernel": plan.info(g3.G3_INFO_KERNEL), "launches": plan.info(g3.G3_INFO_KERNEL_LAUNCHES)}
+        return counts.cpu().numpy().view(np.uint64), g3v.cpu().numpy(), stats, info
+
+
+def check(oracle_lib, g3, pos, box, r_max, n_r, n_t, mode="cells", **opts):
+    H, G, stats, info = run_gpu(g3, pos, box, r_max, n_r, n_t, **opts)
+    pos3 = pos if pos.ndim == 3 else pos[None]
+    orc = oracle_lib.Oracle(pos3.shape[1], box, r_max, n_r, n_t, mode=mode)
+    orc.accumulate(pos3)
+    Ho, Go, so = orc.finalize()
+    assert stats == [int(v) for v in so]
+    assert np.array_equal(H, Ho)
+    nz = Go != 0
+    assert np.array_equal(nz, G != 0)
+    assert np.allclose(G[nz], Go[nz], rtol=G3_RTOL, atol=0)
+    assert info["launches"] > 0
+    return H, stats, info
+
+
+KERNELS = [1]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("widx,nf", [(1, 10), (2, 3), (3, 2), (4, 2)])
+def test_workload_frames(oracle_lib, g3, widx, nf, kernel):
+    w = WORKLOADS[widx]
+    _, pos = frames(w, nf)
+    H, stats, _ = check(oracle_lib, g3, pos, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
+    assert H.sum() > 0 and stats[2] == 0
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config5_one_frame(oracle_lib, g3, kernel):
+    w = WORKLOADS[5]
+    _, pos = frames(w, 1)
+    check(oracle_lib, g3, pos, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("n,box,r_max,n_r,n_t", [
+    (3, 1.0, 0.4, 4, 4),            # smallest legal frame
+    (37, 6.0, 2.9, 8, 16),          # degenerate cell grid (r_max ~ box/2), ragged warp tail
+    (1000, 10.0, 2.0, 7, 13),       # odd bin counts, ncell = 4..5
+    (5000, 10.0, 0.35, 33, 66),     # sparse: many centres with 0 or 1 neighbours
+])
+def test_edge_shapes(oracle_lib, g3, n, box, r_max, n_r, n_t, kernel):
+    m = uniform_frame(n, seed=4242 + n)
+    if n == 3:
+        m = np.array([[5, 5, 5], [5 + GRID // 4, 5, 5], [5, 5 + GRID // 4, 5]], dtype=np.int32)
+    check(oracle_lib, g3, grid_to_pos(m, box), box, r_max, n_r, n_t, mode="allpairs", kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_clumped_and_coincident(oracle_lib, g3, kernel):
+    """all particles in a small blob straddling the periodic corner; two coincident particles"""
+    rng = np.random.default_rng(99)
+    m = ((rng.integers(0, GRID // 16, size=(300, 3)) - GRID // 32) % GRID).astype(np.int32)
+    m[1] = m[0]
+    check(oracle_lib, g3, grid_to_pos(m, 8.0), 8.0, 0.3, 16, 16, mode="allpairs", kernel=kernel,
+          max_neighbours=320)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_off_grid_and_unwrapped_inputs(oracle_lib, g3, kernel):
+    """any real coordinate is snapped to the grid and wrapped (include/g3.h)"""
+    w = WORKLOADS[1]
+    _, pos = frames(w, 2)
+    rng = np.random.default_rng(5)
+    messy = pos + rng.integers(-3, 4, size=pos.shape) * w.box + 0.2 * w.box / GRID
+    H1, _, _, _ = run_gpu(g3, pos, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
+    H2, _, _, _ = run_gpu(g3, messy, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
+    assert np.array_equal(H1, H2)
+    check(oracle_lib, g3, messy, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_batching_single_frame_calls_and_reset(oracle_lib, g3, kernel):
+    """frame-at-a-time calls, batch sizes that do not divide the frame count, finalize twice, reset"""
+    import torch
+    w = WORKLOADS[2]
+    _, pos = frames(w, 7)
+    orc = oracle_lib.Oracle(w.n, w.box, w.r_max, w.n_r, w.n_t, mode="cells")
+    orc.accumulate(pos)
+    Ho, _, so = orc.finalize()
+    d = torch.from_numpy(pos).cuda()
+    for batch in (1, 3, 16):
+        with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, batch_frames=batch, kernel=kernel) as plan:
+            for f in range(4):
+                plan.accumulate_frame(d[f])
+            c1, _, s1 = plan.finalize(want_g3=False)
+            plan.accumulate_frames(d[4:])
+            c2, _, s2 = plan.finalize(want_g3=False)
+            c3, _, s3 = plan.finalize(want_g3=False)
+            assert s1[0] == 4 and s2 == [int(v) for v in so] and s3 == s2
+            assert np.array_equal(c2.cpu().numpy().view(np.uint64), Ho)
+            assert torch.equal(c2, c3)
+            plan.reset()
+            plan.accumulate_frames(d[:4])
+            c4, _, s4 = plan.finalize(want_g3=False)
+            assert torch.equal(c4, c1) and s4 == s1
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_host_entry_points(oracle_lib, g3, kernel):
+    import torch
+    w = WORKLOADS[2]
+    _, pos = frames(w, 5)
+    orc = oracle_lib.Oracle(w.n, w.box, w.r_max, w.n_r, w.n_t, mode="cells")
+    orc.accumulate(pos)
+    Ho, Go, so = orc.finalize()
+    h = torch.from_numpy(pos).pin_memory()
+    with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, batch_frames=2, kernel=kernel) as plan:
+        plan.accumulate_frames_host(h)
+        counts, g3v, stats = plan.finalize_host()
+        assert stats == [int(v) for v in so]
+        assert np.array_equal(counts.numpy().view(np.uint64), Ho)
+        nz = Go != 0
+        assert np.allclose(g3v.numpy()[nz], Go[nz], rtol=G3_RTOL, atol=0)
+        V = plan.bin_volumes()
+        Vo = oracle_lib.volumes(w.r_max, w.n_r, w.n_t)
+        assert np.array_equal(V > 0, Vo > 0)
+        assert np.allclose(V[V > 0], Vo[V > 0], rtol=5e-13, atol=0)
+
+
+def test_capacity_error_is_reported(g3):
+    import torch
+    m = uniform_frame(2000, seed=1)
+    pos = grid_to_pos(m, 10.0)
+    with g3.Plan(2000, 10.0, 2.0, 8, 8, max_neighbours=32, kernel=1) as plan:
+        plan.accumulate_frames(torch.from_numpy(pos[None]).cuda())
+        with pytest.raises(g3.G3Error) as e:
+            plan.finalize()
+        assert e.value.code == g3.G3_ECAPACITY
+
+
+def test_normalize_merged_counts(oracle_lib, g3):
+    """frame-sharded merge: counts from two plans summed, then g3_normalize"""
+    import torch
+    w = WORKLOADS[1]
+    _, pos = frames(w, 6)
+    d = torch.from_numpy(pos).cuda()
+    with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t) as pa, g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t) as pb:
+        pa.accumulate_frames(d[0::2].contiguous())
+        pb.accumulate_frames(d[1::2].contiguous())
+        ca, _, sa = pa.finalize(want_g3=False)
+        cb, _, sb = pb.finalize(want_g3=False)
+        g = pa.normalize(ca + cb, sa[0] + sb[0])
+        torch.cuda.synchronize()
+    orc = oracle_lib.Oracle(w.n, w.box, w.r_max, w.n_r, w.n_t)
+    orc.accumulate(pos)
+    Ho, Go, _ = orc.finalize()
+    assert np.array_equal((ca + cb).cpu().numpy().view(np.uint64), Ho)
+    nz = Go != 0
+    assert np.allclose(g.cpu().numpy()[nz], Go[nz], rtol=G3_RTOL, atol=0)
