@@ -55,7 +55,7 @@ void free_buffers(g3_plan* p) {
     cudaFree(p->d_cell_start); p->d_cell_start = nullptr;
     cudaFree(p->d_sorted); p->d_sorted = nullptr;
     cudaFree(p->d_h2d); p->d_h2d = nullptr;
-    cudaFree(p->d_tiled_scratch); p->d_tiled_scratch = nullptr;
+    tiled_free(p);
     p->configured = false;
 }
 
@@ -67,8 +67,8 @@ int configure(g3_plan* p) {
     int64_t ncell = kGrid / reach;                         // cell width >= reach
     ncell = std::min<int64_t>(ncell, kMaxCellsPerEdge);
     // do not build cells far finer than the particle spacing
-    while (ncell > 3 && ncell * ncell * ncell > 4 * p->n) --ncell;
-    if (ncell < 3) ncell = 1;                              // degenerate grid: all-pairs candidates
+    while (ncell > 4 && ncell * ncell * ncell > 4 * p->n) --ncell;
+    if (ncell < 4) ncell = 1;     // degenerate grid (27 cells would cover the box): all particles
     p->ncell = (int32_t)ncell;
 
     const double frac = p->r_max / p->box;
@@ -219,7 +219,6 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
         if (p->T_t[i] >= p->T_t[i + 1]) { delete p; return G3_EINVAL; }
     if (!bin_volumes(r_max, bins.n_r, bins.n_t, p->volumes)) { delete p; return G3_EINVAL; }
 
-    int rc = G3_OK;
     auto fail = [&](int code) { g3_plan_destroy(p); return code; };
 #define G3_TRY(call)                                                           \
     do {                                                                       \
@@ -240,7 +239,6 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
     G3_TRY(cudaMemset(p->d_counts, 0, sizeof(unsigned long long) * p->nbins));
     G3_TRY(cudaMemset(p->d_stats, 0, sizeof(unsigned long long) * 4));
 #undef G3_TRY
-    (void)rc;
     *out = p;
     return G3_OK;
 }
@@ -355,6 +353,8 @@ int g3_finalize(g3_plan* p, uint64_t* d_counts, double* d_g3, uint64_t* h_stats,
     if (rc != G3_OK) return rc;
     rc = flush(p, st);
     if (rc != G3_OK) return rc;
+    rc = tiled_merge(p, st);
+    if (rc != G3_OK) return rc;
     if (d_counts)
         G3_CUDA(cudaMemcpyAsync(d_counts, p->d_counts, sizeof(uint64_t) * p->nbins,
                                 cudaMemcpyDeviceToDevice, st));
@@ -400,6 +400,11 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     if (p->configured && p->pending) {
         const size_t nc3 = (size_t)p->ncell * p->ncell * p->ncell;
         G3_CUDA(cudaMemsetAsync(p->d_cell_count, 0, sizeof(int32_t) * p->batch_frames * nc3, st));
+    }
+    if (p->tiled) {
+        G3_CUDA(cudaMemsetAsync(p->tiled->d_scratch, 0,
+                                sizeof(uint32_t) * p->tiled->tile_bins * p->tiled->grid, st));
+        p->tiled->frames_since_merge = 0;
     }
     p->pending = 0;
     p->frames = 0;

@@ -33,6 +33,8 @@ struct BinSpec {
 
 }  // namespace g3
 
+namespace g3 { struct TiledState; }
+
 struct g3_plan {
     // problem
     int64_t n = 0;
@@ -71,8 +73,7 @@ struct g3_plan {
     double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
     cudaEvent_t h2d_done[2] = {nullptr, nullptr};
     int64_t h2d_chunk_frames = 0;
-    void* d_tiled_scratch = nullptr;         // owned by the tiled kernel (work counters etc.)
-    size_t tiled_scratch_bytes = 0;
+    g3::TiledState* tiled = nullptr;         // owned by the tiled kernel path (g3_tiled.cuh)
 
     // state
     int32_t pending = 0;                     // frames staged, not yet reduced

@@ -46,10 +46,12 @@ def check(oracle_lib, g3, pos, box, r_max, n_r, n_t, mode="cells", **opts):
     assert np.array_equal(nz, G != 0)
     assert np.allclose(G[nz], Go[nz], rtol=G3_RTOL, atol=0)
     assert info["launches"] > 0
+    if "kernel" in opts and opts["kernel"] in (1, 2) and opts.get("expect_kernel", True):
+        pass
     return H, stats, info
 
 
-KERNELS = [1]
+KERNELS = [1, 2]
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
