@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the g(3) hot path (libg3, include/g3.h) on BASELINE.json's headline
+workload: config 4, N = 32768 water-like sites, 500 frames, r_max = 0.7 nm, 64^3 bins.
+
+A "step" is one pass of the WHOLE hot path (quantise, cell list, neighbour lists, triplet
+histogram, merge, normalise: SURVEY.md 8(a) rows a1..a6) over one seeded synthetic trajectory
+of `--frames` frames (default: the workload's 500).  The metric is distinct triplets binned per
+second (frames/s is reported beside it).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--frames F]
+
+Prints ONE JSON line (rank 0).  `value` is device-timed with positions resident in HBM; `e2e` is
+the same step through the C ABI's host entry points (pinned host positions in, host results out,
+copies inside the timed region).  `roofline` and `cpu_baseline` are described in DESIGN.md 6.
+With --gpus N > 1 (torchrun) every rank processes its own trajectory of the same shape
+(frames are independent; "split the trajectory, merge the results",
+PAPER.md:356, 727): weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import WORKLOADS, frame_iter, grid_to_pos  # noqa: E402
+
+METRIC = "g3_distinct_triplets_binned_per_s"
+UNIT = "triplets/s"
+WORKLOAD_INDEX = 4
+ALGO_INSTR_PER_TRIPLET = 12          # fixed algorithmic instruction count
+SM_LANES = 128                       # 4 schedulers x 32 lanes, one warp instruction per cycle each
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.1 and len(r) >= 7] or \
+               [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower() == "active" for r in rows)]
+
+        def num(s):
+            try:
+                return float(s)
+            except ValueError:
+                return float("nan")
+        return {"sm_mhz": statistics.median(num(r[0]) for r in rows), "sm_max_mhz": num(rows[0][1]),
+                "power_w_max": max(num(r[2]) for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+def make_positions(w, n_frames: int, rank: int) -> np.ndarray:
+    """fp64 [F, n, 3] seeded synthetic frames (workloads/frames.py); rank r > 0 gets its own seed."""
+    ms = list(frame_iter(w, n_frames, seed=w.seed + 1000 * rank))
+    return grid_to_pos(np.stack(ms, axis=0), w.box)
+
+
+def cpu_baseline_leg(w, budget_s: float = 20.0):
+    """The oracle as it stands (oracle/g3_oracle.c, cell-grid routine, OpenMP over centres) on a
+    bounded sample: whole frames of the same workload until ~budget_s of CPU time is spent."""
+    import oracle
+    oracle.build()
+    T_r, T_t = oracle.thresholds(w.box, w.r_max, w.n_r, w.n_t)
+    H = np.zeros((w.n_r, w.n_r, w.n_t), dtype=np.uint64)
+    stats = np.zeros(3, dtype=np.uint64)
+    done, t0 = 0, time.perf_counter()
+    for m in frame_iter(w, w.n_frames):
+        oracle.frame_cells(m, T_r, T_t, H, stats)
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    triplets = (int(stats[1]) + 0) // 2
+    return {"value": triplets / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"first {done} frame(s) of {w.name} ({triplets} distinct triplets), "
+                      f"frame generation included, {dt:.1f} s wall",
+            "frames_per_s": done / dt}, done, dt, triplets
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores, same metric and config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = WORKLOADS[WORKLOAD_INDEX]
+    import oracle
+    oracle.build()
+    T_r, T_t = oracle.thresholds(w.box, w.r_max, w.n_r, w.n_t)
+    frames_per_step = max(1, args.ref_frames)
+    need = frames_per_step * (args.steps + args.warmup)
+    ms = list(frame_iter(w, min(need, w.n_frames)))
+    H = np.zeros((w.n_r, w.n_r, w.n_t), dtype=np.uint64)
+    stats = np.zeros(3, dtype=np.uint64)
+    V = oracle.volumes(w.r_max, w.n_r, w.n_t)
+    k = 0
+
+    def step():
+        nonlocal k
+        for _ in range(frames_per_step):
+            oracle.frame_cells(ms[k % len(ms)], T_r, T_t, H, stats)
+            k += 1
+        oracle.normalise(H, V, int(stats[0]), w.n, w.box)
+
+    for _ in range(args.warmup):
+        step()
+    before = int(stats[1])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    triplets = (int(stats[1]) - before) // 2
+    value = triplets / dt
+    sample = f"{frames_per_step} frame(s) of {w.name} per step ({triplets // args.steps} distinct triplets)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+        "data": "synthetic", "frames_per_s": frames_per_step * args.steps / dt,
+        "config": {"workload": f"config4 {w.name}: N={w.n}, L={w.box}, r_max={w.r_max}, "
+                               f"{w.n_r}x{w.n_r}x{w.n_t} bins; bounded sample: {sample}"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libg3 has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_1708_08619_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1708_08619_b200 as g3
+    from paper_1708_08619_b200.sharding import merge_counts
+
+    w = WORKLOADS[WORKLOAD_INDEX]
+    F = args.frames or w.n_frames
+    pos = make_positions(w, F, rank)                                  # fp64 [F, n, 3]
+    h_pos = torch.from_numpy(pos).pin_memory()
+    d_pos = h_pos.cuda(non_blocking=True)
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+
+    plan = g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, timing=True,
+                   batch_frames=args.batch_frames or None)
+
+    def step_device():
+        plan.reset()
+        plan.accumulate_frames(d_pos)
+        counts, _, stats = plan.finalize(want_g3=False)
+        if world > 1:
+            counts = merge_counts(counts)            # one sum of the 2 MiB histogram per run
+        g = plan.normalize(counts, stats[0] * world)
+        return counts, g, stats
+
+    def step_host():
+        plan.reset()
+        plan.accumulate_frames_host(h_pos)
+        return plan.finalize_host()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        """(ms per step as the max over ranks, last result); CUDA events on the launching stream."""
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.time()
+        e0.record(stream)
+        out = None
+        for _ in range(steps):
+            out = fn()
+        e1.record(stream)
+        barrier()
+        t1 = time.time()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item()) / steps, out, t0, t1
+
+    for _ in range(max(args.warmup, 3)):
+        step_device()
+    plan.clear_timing()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ms_dev, (counts, g, stats), t0, t1 = timed(step_device, args.steps)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    launches = plan.info(g3.G3_INFO_KERNEL_LAUNCHES) // args.steps
+    tri_ns = plan.info(g3.G3_INFO_TRIPLET_NS)
+    nb_ns = plan.info(g3.G3_INFO_NEIGHBOUR_NS)
+    tri_launches = plan.info(g3.G3_INFO_TIMED_LAUNCHES)
+    triplets_rank = (stats[1] + stats[2]) // 2                         # distinct triplets per step
+    tot = torch.tensor([triplets_rank], dtype=torch.int64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tot)
+    triplets_all = int(tot.item())
+
+    for _ in range(2):
+        step_host()
+    ms_e2e, (h_counts, h_g3, h_stats), _, _ = timed(step_host, args.steps)
+    assert h_stats[1] == stats[1], "host and device entry points disagree"
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    pk, pk_kind = peaks()
+    sm_count = plan.info(g3.G3_INFO_SM_COUNT)
+    sm_hz = float(pk.get("sm_max_mhz", 1965.0)) * 1e6
+    peak_tinstr = sm_count * SM_LANES * sm_hz / 1e12
+    tri_s = tri_ns * 1e-9 / max(tri_launches, 1)                       # avg triplet-kernel launch
+    trip_per_launch = triplets_rank * args.steps / max(tri_launches, 1)
+    achieved = trip_per_launch * ALGO_INSTR_PER_TRIPLET / tri_s / 1e12 if tri_s > 0 else 0.0
+    roofline = {
+        "bound": "alu", "kernel": "tiled_triplet_kernel", "achieved": achieved, "peak": peak_tinstr,
+        "unit": "Tinstr/s", "frac": achieved / peak_tinstr, "traffic": None,
+        "peak_kind": f"{sm_count} SMs x {SM_LANES} lanes x sm_max_mhz ({pk_kind}); DESIGN.md 6",
+        "algorithmic_instr_per_triplet": ALGO_INSTR_PER_TRIPLET,
+        "triplets_per_launch": trip_per_launch, "kernel_ms_per_launch": tri_s * 1e3,
+        "kernel_launches_per_step": tri_launches / args.steps,
+        "kernel_share_of_step": tri_ns * 1e-6 / args.steps / ms_dev,
+        "neighbour_kernel_share_of_step": nb_ns * 1e-6 / args.steps / ms_dev,
+        "kernel_triplets_per_s": trip_per_launch / tri_s if tri_s > 0 else 0.0,
+        "whole_step_frac": triplets_rank / (ms_dev * 1e-3) * ALGO_INSTR_PER_TRIPLET / 1e12 / peak_tinstr,
+        "hbm_gbs_achieved_step": F * w.n * 24 / (ms_dev * 1e-3) / 1e9,
+        "hbm_gbs_peak": pk.get("hbm_gbs"),
+    }
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu, _, _, _ = cpu_baseline_leg(w, args.cpu_budget)
+    nbytes = w.n_r * w.n_r * w.n_t * 8
+    line = {
+        "metric": METRIC, "value": triplets_all / (ms_dev * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_dev,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+int64",
+        "data": "synthetic", "frames_per_s": F * world / (ms_dev * 1e-3),
+        "config": {"workload": f"config4 {w.name}: N={w.n}, L={w.box}, r_max={w.r_max}, "
+                               f"{w.n_r}x{w.n_r}x{w.n_t} bins, {F} frames per step per GPU",
+                   "frames_per_step": F, "triplets_per_step": triplets_all,
+                   "batch_frames": plan.info(g3.G3_INFO_BATCH_FRAMES),
+                   "kernel": plan.info(g3.G3_INFO_KERNEL),
+                   "l2": f"inputs larger than L2 ({F * w.n * 24 / 2**20:.0f} MiB of positions per step)",
+                   "parallelism": f"frames sharded over {world} GPU(s), one histogram sum per run"},
+        "clocks": clocks,
+        "e2e": {"value": triplets_all / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                "frames_per_s": F * world / (ms_e2e * 1e-3),
+                "h2d_bytes_per_step": F * w.n * 24, "d2h_bytes_per_step": 2 * nbytes + 24},
+        "gpu_launches": launches * args.steps,
+        "gpu_launches_per_step": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--frames", type=int, default=0, help="frames per step (default: the workload's)")
+    ap.add_argument("--batch-frames", type=int, default=0)
+    ap.add_argument("--ref-frames", type=int, default=4, help="frames per step of --impl reference")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

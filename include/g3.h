@@ -78,19 +78,26 @@ typedef enum {
 typedef enum {
     G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1)      */
     G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
-    G3_OPT_MAX_NEIGHBOURS = 3 /* per-centre neighbour capacity (0 = derive from density)     */
+    G3_OPT_MAX_NEIGHBOURS = 3, /* per-centre neighbour capacity (0 = derive from density)    */
+    G3_OPT_TIMING = 4         /* 1 = bracket the neighbour and triplet kernels with CUDA events
+                                 on the caller's stream (read back with g3_plan_get_info)     */
 } g3_option;
 
 /* Keys for g3_plan_get_info. */
 typedef enum {
-    G3_INFO_KERNEL_LAUNCHES = 1, /* kernels launched by this plan since creation / reset     */
+    G3_INFO_KERNEL_LAUNCHES = 1, /* kernels launched since creation / g3_plan_clear_timing    */
     G3_INFO_BATCH_FRAMES = 2,
     G3_INFO_KERNEL = 3,          /* kernel actually selected (1 or 2)                        */
     G3_INFO_CELLS_PER_EDGE = 4,
     G3_INFO_MAX_NEIGHBOURS = 5,
     G3_INFO_TILE_BINS = 6,       /* histogram bins privatised in shared memory per CTA       */
     G3_INFO_SM_COUNT = 7,
-    G3_INFO_FRAMES_PENDING = 8   /* staged frames not yet reduced into the histogram         */
+    G3_INFO_FRAMES_PENDING = 8,  /* staged frames not yet reduced into the histogram         */
+    /* G3_OPT_TIMING = 1 only.  Reading any of the three waits for the recorded events; the
+     * sums cover the launches since creation or the last g3_plan_clear_timing.             */
+    G3_INFO_TRIPLET_NS = 9,      /* device time of the triplet kernel launches, nanoseconds  */
+    G3_INFO_NEIGHBOUR_NS = 10,   /* device time of the neighbour kernel launches             */
+    G3_INFO_TIMED_LAUNCHES = 11  /* launches of EACH of the two kernels covered by the sums  */
 } g3_info;
 
 /* Create a plan for frames of `n` particles in a cubic periodic box of edge `box`
@@ -110,6 +117,9 @@ G3_API int g3_plan_create(g3_plan **out, int64_t n, double box, double r_max, g3
  * (until g3_plan_reset), G3_EINVAL for unknown keys or bad values.                  */
 G3_API int g3_plan_set_option(g3_plan *p, int32_t option, int64_t value);
 G3_API int g3_plan_get_info(const g3_plan *p, int32_t key, int64_t *value);
+
+/* Forget the kernel times and the launch counter gathered so far (histogram untouched).  */
+G3_API int g3_plan_clear_timing(g3_plan *p);
 
 /* Add one frame (Algorithm 6/7's loop body).
  *   d_pos  device, fp64, [n][3] row-major (x,y,z of particle 0, then particle 1, ...).

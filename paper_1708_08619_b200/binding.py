@@ -14,12 +14,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libg3.so")
 
 G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
-G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS = 1, 2, 3
+G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING = 1, 2, 3, 4
 (G3_INFO_KERNEL_LAUNCHES, G3_INFO_BATCH_FRAMES, G3_INFO_KERNEL, G3_INFO_CELLS_PER_EDGE,
- G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING) = range(1, 9)
+ G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING,
+ G3_INFO_TRIPLET_NS, G3_INFO_NEIGHBOUR_NS, G3_INFO_TIMED_LAUNCHES) = range(1, 12)
 
 EXPORTS = [
-    "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_accumulate_frame",
+    "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
+    "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
     "g3_normalize", "g3_bin_volumes", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
@@ -51,6 +53,7 @@ def load() -> C.CDLL:
     lib.g3_plan_create.argtypes = [C.POINTER(vp), i64, f64, f64, g3_bins]
     lib.g3_plan_set_option.argtypes = [vp, i32, i64]
     lib.g3_plan_get_info.argtypes = [vp, i32, C.POINTER(i64)]
+    lib.g3_plan_clear_timing.argtypes = [vp]
     lib.g3_accumulate_frame.argtypes = [vp, vp, vp]
     lib.g3_accumulate_frames.argtypes = [vp, vp, i64, i64, vp]
     lib.g3_accumulate_frames_host.argtypes = [vp, vp, i64, i64, vp]
@@ -92,7 +95,7 @@ class Plan:
 
     def __init__(self, n: int, box: float, r_max: float, n_r: int, n_t: Optional[int] = None, *,
                  batch_frames: Optional[int] = None, kernel: Optional[int] = None,
-                 max_neighbours: Optional[int] = None):
+                 max_neighbours: Optional[int] = None, timing: bool = False):
         self._lib = load()
         self.n, self.box, self.r_max = int(n), float(box), float(r_max)
         self.n_r, self.n_t = int(n_r), int(n_r if n_t is None else n_t)
@@ -105,6 +108,8 @@ class Plan:
             self.set_option(G3_OPT_KERNEL, kernel)
         if max_neighbours is not None:
             self.set_option(G3_OPT_MAX_NEIGHBOURS, max_neighbours)
+        if timing:
+            self.set_option(G3_OPT_TIMING, 1)
 
     # -- options / info -------------------------------------------------------------------
     def set_option(self, option: int, value: int) -> None:
@@ -114,6 +119,9 @@ class Plan:
         v = C.c_int64()
         _check(self._lib.g3_plan_get_info(self._h, key, C.byref(v)), "g3_plan_get_info")
         return int(v.value)
+
+    def clear_timing(self) -> None:
+        _check(self._lib.g3_plan_clear_timing(self._h), "g3_plan_clear_timing")
 
     @property
     def shape(self) -> Tuple[int, int, int]:

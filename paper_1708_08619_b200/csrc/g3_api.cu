@@ -59,6 +59,21 @@ void free_buffers(g3_plan* p) {
     p->configured = false;
 }
 
+// Fold the recorded event triples into the running sums (waits for the last event).
+int fold_timing(g3_plan* p) {
+    for (size_t i = 0; i + 2 < p->ev_used; i += 3) {
+        float nb = 0.f, tri = 0.f;
+        G3_CUDA(cudaEventSynchronize(p->ev_pool[i + 2]));
+        G3_CUDA(cudaEventElapsedTime(&nb, p->ev_pool[i], p->ev_pool[i + 1]));
+        G3_CUDA(cudaEventElapsedTime(&tri, p->ev_pool[i + 1], p->ev_pool[i + 2]));
+        p->neighbour_ms += nb;
+        p->triplet_ms += tri;
+        p->timed_launches += 1;
+    }
+    p->ev_used = 0;
+    return G3_OK;
+}
+
 // Choose the cell grid, the neighbour capacity and the kernel; allocate batch buffers.
 int configure(g3_plan* p) {
     if (p->configured) return G3_OK;
@@ -256,6 +271,9 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
         case G3_OPT_MAX_NEIGHBOURS:
             if (value < 0 || value > (1 << 20)) return G3_EINVAL;
             p->max_nb_opt = (int32_t)value; break;
+        case G3_OPT_TIMING:
+            if (value < 0 || value > 1) return G3_EINVAL;
+            p->timing = (int32_t)value; return G3_OK;
         default: return G3_EINVAL;
     }
     if (p->configured) free_buffers(p);
@@ -265,6 +283,14 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
 int g3_plan_get_info(const g3_plan* cp, int32_t key, int64_t* value) {
     if (!cp || !value) return G3_EINVAL;
     g3_plan* p = const_cast<g3_plan*>(cp);
+    if (key >= G3_INFO_TRIPLET_NS && key <= G3_INFO_TIMED_LAUNCHES) {
+        int rc = fold_timing(p);
+        if (rc != G3_OK) return rc;
+        *value = key == G3_INFO_TRIPLET_NS ? (int64_t)llround(p->triplet_ms * 1e6)
+               : key == G3_INFO_NEIGHBOUR_NS ? (int64_t)llround(p->neighbour_ms * 1e6)
+               : p->timed_launches;
+        return G3_OK;
+    }
     if (key != G3_INFO_KERNEL_LAUNCHES && key != G3_INFO_FRAMES_PENDING && key != G3_INFO_SM_COUNT &&
         key != G3_INFO_BATCH_FRAMES) {
         int rc = configure(p);
@@ -282,6 +308,15 @@ int g3_plan_get_info(const g3_plan* cp, int32_t key, int64_t* value) {
         default: return G3_EINVAL;
     }
     return G3_OK;
+}
+
+int g3_plan_clear_timing(g3_plan* p) {
+    if (!p) return G3_EINVAL;
+    int rc = fold_timing(p);
+    p->triplet_ms = p->neighbour_ms = 0;
+    p->timed_launches = 0;
+    p->launches = 0;
+    return rc;
 }
 
 int g3_accumulate_frames(g3_plan* p, const double* d_pos, int64_t n_frames, int64_t frame_stride,
@@ -408,7 +443,6 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     }
     p->pending = 0;
     p->frames = 0;
-    p->launches = 0;
     return G3_OK;
 }
 
@@ -418,6 +452,7 @@ void g3_plan_destroy(g3_plan* p) {
     free_buffers(p);
     for (int i = 0; i < 2; ++i)
         if (p->h2d_done[i]) cudaEventDestroy(p->h2d_done[i]);
+    for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
     cudaFree(p->d_T_r); cudaFree(p->d_T_t); cudaFree(p->d_counts); cudaFree(p->d_stats);
     cudaFree(p->d_volumes);
     cudaGetLastError();

@@ -57,6 +57,7 @@ struct g3_plan {
     int32_t ncell = 1;
     int32_t max_nb = 0;                      // neighbour capacity per centre
     int32_t max_nb_opt = 0;
+    int32_t timing = 0;                      // G3_OPT_TIMING
     int64_t tile_bins = 0;
 
     // device buffers
@@ -73,6 +74,11 @@ struct g3_plan {
     double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
     cudaEvent_t h2d_done[2] = {nullptr, nullptr};
     int64_t h2d_chunk_frames = 0;
+    // G3_OPT_TIMING: event triples (before neighbour, between, after triplet) per launch pair
+    std::vector<cudaEvent_t> ev_pool;        // all events ever created (reused after a clear)
+    size_t ev_used = 0;                      // events of ev_pool recorded since the last clear
+    double triplet_ms = 0, neighbour_ms = 0; // sums already folded in
+    int64_t timed_launches = 0;
     g3::TiledState* tiled = nullptr;         // owned by the tiled kernel path (g3_tiled.cuh)
 
     // state

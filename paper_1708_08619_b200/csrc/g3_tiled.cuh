@@ -624,6 +624,18 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     np.T_r = bs.T_r; np.addend = ts->d_addend; np.jconst = ts->d_jconst;
     np.nbv = ts->d_nbv; np.nbj = ts->d_nbj; np.nbcount = ts->d_nbcount; np.stats = p->d_stats;
     G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    if (p->timing) {
+        for (int i = 0; i < 3; ++i) {
+            if (p->ev_used == p->ev_pool.size()) {
+                cudaEvent_t e;
+                G3T_CUDA(cudaEventCreate(&e));
+                p->ev_pool.push_back(e);
+            }
+            ev[i] = p->ev_pool[p->ev_used++];
+        }
+        G3T_CUDA(cudaEventRecord(ev[0], st));
+    }
     if (fb.ncell == 1) {
         dim3 grid((unsigned)fb.n_frames, (unsigned)((fb.n + 63) / 64));
         neighbour_kernel<true><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
@@ -631,6 +643,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         dim3 grid((unsigned)((long long)fb.n_frames * fb.ncell3), 1);
         neighbour_kernel<false><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
     }
+    if (p->timing) G3T_CUDA(cudaEventRecord(ev[1], st));
     TriParams tp;
     tp.total_centres = (long long)fb.n_frames * fb.n;
     tp.max_nb = p->max_nb; tp.n_t = bs.n_t; tp.tile_bins = (int32_t)ts->tile_bins;
@@ -644,6 +657,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         case 16: tiled_triplet_kernel<16><<<ts->grid, 16 * 32, ts->tri_smem, st>>>(tp); break;
         default: tiled_triplet_kernel<8><<<ts->grid, 8 * 32, ts->tri_smem, st>>>(tp); break;
     }
+    if (p->timing) G3T_CUDA(cudaEventRecord(ev[2], st));
     p->launches += 2;
     ts->frames_since_merge += fb.n_frames;
     G3T_CUDA(cudaGetLastError());

@@ -116,12 +116,14 @@ def _chain_sites(w: Workload, rng: np.random.Generator) -> np.ndarray:
     return pos.reshape(-1, 3)
 
 
-def frame_iter(w: Workload, n_frames: Optional[int] = None) -> Iterator[np.ndarray]:
-    """Yield int32 [n, 3] grid coordinates, frame after frame, from the config's seed.
+def frame_iter(w: Workload, n_frames: Optional[int] = None,
+               seed: Optional[int] = None) -> Iterator[np.ndarray]:
+    """Yield int32 [n, 3] grid coordinates, frame after frame, from the config's seed
+    (or from `seed`: a different trajectory of the same recipe, e.g. one per rank).
 
     The first `k` frames are the same whatever `n_frames` is asked for."""
     total = w.n_frames if n_frames is None else int(n_frames)
-    rng = np.random.default_rng(w.seed)
+    rng = np.random.default_rng(w.seed if seed is None else seed)
     if w.kind == "uniform":
         for _ in range(total):
             yield rng.integers(0, GRID, size=(w.n, 3), dtype=np.int64).astype(np.int32)
