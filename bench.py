@@ -209,7 +209,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     plan = g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, timing=True,
-                   batch_frames=args.batch_frames or None)
+                   batch_frames=args.batch_frames or None, triplet_warps=args.triplet_warps or None)
 
     def step_device():
         plan.reset()
@@ -337,6 +337,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--frames", type=int, default=0, help="frames per step (default: the workload's)")
     ap.add_argument("--batch-frames", type=int, default=0)
+    ap.add_argument("--triplet-warps", type=int, default=0)
     ap.add_argument("--ref-frames", type=int, default=4, help="frames per step of --impl reference")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

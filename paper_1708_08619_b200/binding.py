@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libg3.so")
 
 G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
-G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING = 1, 2, 3, 4
+G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING, G3_OPT_TRIPLET_WARPS = 1, 2, 3, 4, 5
 (G3_INFO_KERNEL_LAUNCHES, G3_INFO_BATCH_FRAMES, G3_INFO_KERNEL, G3_INFO_CELLS_PER_EDGE,
  G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING,
  G3_INFO_TRIPLET_NS, G3_INFO_NEIGHBOUR_NS, G3_INFO_TIMED_LAUNCHES) = range(1, 12)
@@ -95,7 +95,8 @@ class Plan:
 
     def __init__(self, n: int, box: float, r_max: float, n_r: int, n_t: Optional[int] = None, *,
                  batch_frames: Optional[int] = None, kernel: Optional[int] = None,
-                 max_neighbours: Optional[int] = None, timing: bool = False):
+                 max_neighbours: Optional[int] = None, timing: bool = False,
+                 triplet_warps: Optional[int] = None):
         self._lib = load()
         self.n, self.box, self.r_max = int(n), float(box), float(r_max)
         self.n_r, self.n_t = int(n_r), int(n_r if n_t is None else n_t)
@@ -110,6 +111,8 @@ class Plan:
             self.set_option(G3_OPT_MAX_NEIGHBOURS, max_neighbours)
         if timing:
             self.set_option(G3_OPT_TIMING, 1)
+        if triplet_warps is not None:
+            self.set_option(G3_OPT_TRIPLET_WARPS, triplet_warps)
 
     # -- options / info -------------------------------------------------------------------
     def set_option(self, option: int, value: int) -> None:

@@ -90,7 +90,7 @@ int configure(g3_plan* p) {
     const double mean_k = (double)p->n * 4.18879020478639 * frac * frac * frac;
     int64_t cap = p->max_nb_opt > 0 ? p->max_nb_opt : (int64_t)(3.0 * mean_k) + 64;
     cap = std::min<int64_t>(cap, p->n - 1);
-    cap = std::max<int64_t>((cap + 31) / 32 * 32, 32);
+    cap = std::max<int64_t>((cap + 31) / 32 * 32, 64);   // >= 64: the triplet kernel prefetches two chunks
     p->max_nb = (int32_t)cap;
 
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled
@@ -271,6 +271,9 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
         case G3_OPT_MAX_NEIGHBOURS:
             if (value < 0 || value > (1 << 20)) return G3_EINVAL;
             p->max_nb_opt = (int32_t)value; break;
+        case G3_OPT_TRIPLET_WARPS:
+            if (value != 0 && value != 8 && value != 16 && value != 24) return G3_EINVAL;
+            p->tri_warps_opt = (int32_t)value; break;
         case G3_OPT_TIMING:
             if (value < 0 || value > 1) return G3_EINVAL;
             p->timing = (int32_t)value; return G3_OK;
@@ -438,8 +441,8 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     }
     if (p->tiled) {
         G3_CUDA(cudaMemsetAsync(p->tiled->d_scratch, 0,
-                                sizeof(uint32_t) * p->tiled->tile_bins * p->tiled->grid, st));
-        p->tiled->frames_since_merge = 0;
+                                sizeof(unsigned long long) * p->tiled->tile_bins * p->tiled->grid, st));
+        p->tiled->dirty = false;
     }
     p->pending = 0;
     p->frames = 0;

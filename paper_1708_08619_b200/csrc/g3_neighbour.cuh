@@ -1,0 +1,232 @@
+// g3_neighbour.cuh -- step a3: minimum-image neighbour lists inside r_max, sorted by shell.
+//
+// Algorithm 7 CUDA_g2 "store minimum image neighbour vectors", done with a cell
+// list instead of the paper's all-particle scan.
+//
+// One CTA (4 warps) per cell.  The particles of the 27 surrounding cells are staged once in
+// shared memory as fp32 coordinates relative to the cell centre (exact: |value| < 2^20), so the
+// minimum-image vector of a neighbour is a plain difference.  A warp per centre then runs
+//   A  a tight scan of the stage: d2 < cut (fp32, widened by 2^-20) -> ballot-compacted list
+//      of (dx, dy, dz, d2) in the warp's shared scratch;
+//   B  per list entry: exact 64-bit test for entries within 2^-20 of the cut-off, shell
+//      a = bin(T_r, d2) (fp32 twice with the scale lowered / raised by 2^-20; 64-bit search in
+//      the exact edge table when the two disagree), rank inside the shell by a shared atomic;
+//   C  exclusive scan of the shell counts and scatter to global memory in shell order:
+//      nbv[centre][pos] = (dx, dy, dz, a).
+// The order inside a shell depends on the atomics' arrival order; the histogram does not.
+#pragma once
+
+#include "g3_generic.cuh"
+#include "g3_plan.h"
+
+namespace g3 {
+
+constexpr float kMagic = 12582912.0f;          // 1.5 * 2^23: fp32 integers with ulp 1 around it
+constexpr uint32_t kMagicBits = 0x4B400000u;
+constexpr int kNbWarps = 4;                    // warps per neighbour_kernel CTA
+constexpr int kMaxRanges = 18;
+
+struct NbParams {
+    int32_t max_nb, stage_cap, n_r;
+    float cut_lo, cut_hi;                 // fp32 window around T_r[n_r]
+    unsigned long long cut2;
+    float inv_w_lo, inv_w_hi;             // (1/w)(1 -+ 2^-20), w = shell width in grid units
+    const unsigned long long* T_r;
+    float4* nbv;                          // [frames][n][max_nb] (dx, dy, dz, shell as int bits)
+    int32_t* nbcount;                     // [frames][n]
+    unsigned long long* stats;
+};
+
+__device__ __forceinline__ float sqrt_approx(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+__device__ __forceinline__ unsigned long long exact_d2(float dx, float dy, float dz) {
+    const long long X = (long long)dx, Y = (long long)dy, Z = (long long)dz;
+    return (unsigned long long)(X * X + Y * Y + Z * Z);
+}
+
+// Phase A for 32 candidates: `c` is this lane's candidate (relative coordinates), `in` says
+// whether it is a real candidate other than the centre itself.
+template <bool kWrap>
+__device__ __forceinline__ void nb_test(float4 c, bool in, float px, float py, float pz,
+                                        float cut_hi, int lane, int32_t max_nb, float4* scratch,
+                                        int32_t& count) {
+    float dx = c.x - px, dy = c.y - py, dz = c.z - pz;
+    if (kWrap) {
+        dx += dx < -524288.f ? 1048576.f : 0.f; dx -= dx >= 524288.f ? 1048576.f : 0.f;
+        dy += dy < -524288.f ? 1048576.f : 0.f; dy -= dy >= 524288.f ? 1048576.f : 0.f;
+        dz += dz < -524288.f ? 1048576.f : 0.f; dz -= dz >= 524288.f ? 1048576.f : 0.f;
+    }
+    const float d2f = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const bool acc = in && d2f < cut_hi;
+    const unsigned mask = __ballot_sync(0xffffffffu, acc);
+    const int32_t pos = count + __popc(mask & ((1u << lane) - 1u));
+    if (acc && pos < max_nb) scratch[pos] = make_float4(dx, dy, dz, d2f);
+    count += __popc(mask);
+}
+
+// kWrap = the cell grid is degenerate (ncell == 1): the stage holds raw coordinates of the whole
+// frame and every difference is wrapped; otherwise the stage is pre-shifted and no wrap is needed.
+template <bool kWrap>
+__global__ void __launch_bounds__(kNbWarps * 32)
+neighbour_kernel(FrameBatch fb, NbParams np) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4* stage = reinterpret_cast<float4*>(smem_raw);
+    float4* scratch_all = stage + np.stage_cap;
+    int32_t* hist_all = reinterpret_cast<int32_t*>(scratch_all + (size_t)kNbWarps * np.max_nb);
+    __shared__ int32_t range_begin[kMaxRanges], range_prefix[kMaxRanges + 1];
+    __shared__ int32_t own_base_s, cell_range[2];
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t f = blockIdx.x / fb.ncell3, cell = blockIdx.x - f * fb.ncell3;
+    const int4* __restrict__ sorted = fb.sorted + (long long)f * fb.n;
+    const int32_t* __restrict__ start = fb.cell_start + (long long)f * (fb.ncell3 + 1);
+
+    // ---- candidate ranges: one lane per range, all loads in flight together --------------------
+    const int32_t n_ranges = CandidateRanges::count(fb.ncell);
+    if (wid == 0) {
+        const int32_t c_begin = kWrap ? 0 : __ldg(start + cell);
+        const int32_t c_end = kWrap ? fb.n : __ldg(start + cell + 1);
+        int32_t b = 0, e = 0;
+        if (lane < n_ranges) CandidateRanges::get(lane, cell, fb.ncell, fb.n, start, b, e);
+        const int32_t len = e - b;
+        int32_t incl = len;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        if (lane < n_ranges) { range_begin[lane] = b; range_prefix[lane] = incl - len; }
+        if (lane == n_ranges - 1) range_prefix[n_ranges] = incl;
+        if (lane < n_ranges && b <= c_begin && c_begin < e) own_base_s = incl - len + (c_begin - b);
+        if (lane == 0) { cell_range[0] = c_begin; cell_range[1] = c_end; }
+    }
+    __syncthreads();
+    const int32_t c_begin = cell_range[0], c_end = cell_range[1];
+    if (c_begin == c_end) return;                         // empty cell: no centres
+    const int32_t n_stage = range_prefix[n_ranges];
+    const bool staged = n_stage <= np.stage_cap;
+    int32_t ox = 0, oy = 0, oz = 0;
+    if (!kWrap) {
+        const int32_t cz = cell % fb.ncell, cy = (cell / fb.ncell) % fb.ncell, cx = cell / (fb.ncell * fb.ncell);
+        ox = (int32_t)(((long long)(2 * cx + 1) << (kGridBits - 1)) / fb.ncell);   // cell centre
+        oy = (int32_t)(((long long)(2 * cy + 1) << (kGridBits - 1)) / fb.ncell);
+        oz = (int32_t)(((long long)(2 * cz + 1) << (kGridBits - 1)) / fb.ncell);
+    }
+    auto relative = [&](int4 c) {
+        if (kWrap) return make_float4((float)c.x, (float)c.y, (float)c.z, 0.f);
+        return make_float4((float)wrap_component(c.x - ox), (float)wrap_component(c.y - oy),
+                           (float)wrap_component(c.z - oz), 0.f);
+    };
+    if (staged) {
+        for (int32_t d = threadIdx.x; d < n_stage; d += blockDim.x) {
+            int32_t r = 0;
+            while (d >= range_prefix[r + 1]) ++r;
+            stage[d] = relative(sorted[range_begin[r] + (d - range_prefix[r])]);
+        }
+        __syncthreads();
+    }
+
+    // ---- one warp per centre -------------------------------------------------------------------
+    float4* scratch = scratch_all + (size_t)wid * np.max_nb;
+    int32_t* hist = hist_all + (size_t)wid * (np.n_r + 1);
+    const int32_t own_base = own_base_s;
+    // degenerate grid: the centres are split over blockIdx.y in slices of 64
+    const int32_t s_lo = kWrap ? min(c_end, (int32_t)blockIdx.y * 64) : c_begin;
+    const int32_t s_hi = kWrap ? min(c_end, (int32_t)(blockIdx.y + 1) * 64) : c_end;
+    unsigned long long my_pairs = 0, my_cap = 0;
+    for (int32_t s = s_lo + wid; s < s_hi; s += kNbWarps) {
+        int32_t count = 0;
+        // phase A
+        if (staged) {
+            const int32_t own = own_base + (s - c_begin);
+            const float4 p = stage[own];
+            for (int32_t q0 = 0; q0 < n_stage; q0 += 32) {
+                const int32_t q = q0 + lane;
+                const bool in = q < n_stage && q != own;
+                const float4 c = in ? stage[q] : p;
+                nb_test<kWrap>(c, in, p.x, p.y, p.z, np.cut_hi, lane, np.max_nb, scratch, count);
+            }
+        } else {                                           // crowded neighbourhood: read from global
+            const float4 p = relative(sorted[s]);
+            for (int32_t r = 0; r < n_ranges; ++r) {
+                const int32_t b = range_begin[r], e = b + (range_prefix[r + 1] - range_prefix[r]);
+                for (int32_t q0 = b; q0 < e; q0 += 32) {
+                    const int32_t q = q0 + lane;
+                    const bool in = q < e && q != s;
+                    const float4 c = in ? relative(sorted[q]) : p;
+                    nb_test<kWrap>(c, in, p.x, p.y, p.z, np.cut_hi, lane, np.max_nb, scratch, count);
+                }
+            }
+        }
+        if (count > np.max_nb) { my_cap += 1; count = np.max_nb; }
+        for (int32_t i = lane; i <= np.n_r; i += 32) hist[i] = 0;
+        __syncwarp();
+
+        // phase B: exact acceptance near the cut-off, shell, rank inside the shell
+        for (int32_t e = lane; e < count; e += 32) {
+            const float4 v = scratch[e];
+            unsigned long long d2 = 0;
+            bool have_exact = false, keep = true;
+            if (v.w > np.cut_lo) {                         // too close to the cut-off for fp32
+                d2 = exact_d2(v.x, v.y, v.z);
+                have_exact = true;
+                keep = d2 < np.cut2;
+            }
+            int32_t a = np.n_r;                            // n_r = rejected
+            if (keep) {
+                const float t = sqrt_approx(v.w);
+                const uint32_t lo = __float_as_uint(__fmaf_rd(t, np.inv_w_lo, kMagic));
+                const uint32_t hi = __float_as_uint(__fmaf_rd(t, np.inv_w_hi, kMagic));
+                if (lo == hi) a = (int32_t)(lo - kMagicBits);
+                else {
+                    if (!have_exact) d2 = exact_d2(v.x, v.y, v.z);
+                    a = bin_search(np.T_r, np.n_r, d2);
+                }
+            }
+            const int32_t rank = atomicAdd(hist + a, 1);
+            scratch[e].w = __int_as_float(a | (rank << 10));
+        }
+        __syncwarp();
+
+        // phase C: exclusive scan of the shell counts, scatter in shell order
+        int32_t carry = 0;
+        for (int32_t i0 = 0; i0 < np.n_r; i0 += 32) {
+            const int32_t i = i0 + lane;
+            const int32_t v = i < np.n_r ? hist[i] : 0;
+            int32_t incl = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            if (i < np.n_r) hist[i] = carry + incl - v;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        __syncwarp();
+        const int32_t kept = carry;
+        my_pairs += (unsigned long long)kept * (unsigned long long)(kept > 0 ? kept - 1 : 0);
+        const long long gbase = ((long long)f * fb.n + s) * np.max_nb;
+        for (int32_t e = lane; e < count; e += 32) {
+            const float4 v = scratch[e];
+            const int32_t packed = __float_as_int(v.w);
+            const int32_t a = packed & 1023, rank = packed >> 10;
+            if (a < np.n_r) np.nbv[gbase + hist[a] + rank] = make_float4(v.x, v.y, v.z, __int_as_float(a));
+        }
+        if (lane == 0) np.nbcount[(long long)f * fb.n + s] = kept;
+        __syncwarp();
+    }
+    if (lane == 0) {
+        if (my_pairs) atomicAdd(np.stats + 0, my_pairs);
+        if (my_cap) atomicAdd(np.stats + 2, my_cap);
+    }
+}
+
+inline size_t nb_smem_bytes(int32_t stage_cap, int32_t max_nb, int32_t n_r) {
+    return (size_t)stage_cap * 16 + (size_t)kNbWarps * max_nb * 16 + (size_t)kNbWarps * (n_r + 1) * 4;
+}
+
+}  // namespace g3

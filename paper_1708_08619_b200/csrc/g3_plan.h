@@ -58,6 +58,7 @@ struct g3_plan {
     int32_t max_nb = 0;                      // neighbour capacity per centre
     int32_t max_nb_opt = 0;
     int32_t timing = 0;                      // G3_OPT_TIMING
+    int32_t tri_warps_opt = 0;               // G3_OPT_TRIPLET_WARPS
     int64_t tile_bins = 0;
 
     // device buffers

@@ -1,0 +1,262 @@
+// g3_triplet.cuh -- steps a4 + a5: the triplet kernel (Algorithm 7 CUDA_g3)
+// and the merge of its per-CTA partial histograms.
+//
+// tiled_triplet_kernel: persistent, one CTA per SM.  A warp per centre; lane = neighbour j
+// (32 at a time), the partner k is broadcast from a 32-entry shared-memory window; every
+// UNORDERED pair j < k is visited once (the lists are sorted by shell, so a_j <= a_k) and
+// counted with one shared-memory atomic into a privatised histogram tile that holds only the
+// bins the triangle inequality allows:
+//     slot(a, b, c) = 1 + BASE(b) + P(a) + c - g(b) + h(a)          (a <= b)
+// (DESIGN.md section 4.3).  Slot 0 is a guard: lanes without a pair in an iteration add to it,
+// so every shared atomic is issued by a full, converged warp (measured on B200: a full-warp
+// ATOMS.POPC.INC retires in 2.0-2.7 SM cycles, a partially predicated one in 4.1 with ~90
+// cycles of latency).  The list of the NEXT centre is loaded into registers while the current
+// one is processed.  When the kernel ends each CTA adds its tile to its own uint64 partial
+// tile in global memory; merge_kernel mirrors the partial tiles into the [a][b][c] histogram.
+//
+// Exactness.  Differences of neighbour vectors are exact in fp32 (integers below 2^21).  The
+// squared distance, its square root and the bin index are computed in fp32 with a relative
+// error below 2^-21; the bin is taken twice, with the scale factor lowered and raised by
+// 2^-20.  If both agree, the exact integer rule bin(T_t, t2) gives the same bin (the exact
+// quotient lies between the two); if they differ the pair is redone in 64-bit integers
+// against the exact edge table and the histogram is corrected.
+#pragma once
+
+#include "g3_neighbour.cuh"
+
+namespace g3 {
+
+constexpr int kItemCentres = 8;                // centres per work-queue fetch
+
+struct TriParams {
+    long long total_centres;              // frames * n
+    int32_t max_nb, n_t, n_r;
+    int32_t tile_bins;
+    uint32_t cta_item_cap;                // items one CTA may take (u32 tile slots cannot overflow)
+    float inv_lo, inv_hi;                 // (1/wt)(1 -+ 2^-20), wt = t-bin width in grid units
+    const unsigned long long* T_t;
+    const float4* nbv;                    // [centres][max_nb] (dx, dy, dz, shell)
+    const int32_t* nbcount;
+    const float* addend;                  // [n_r]  kMagic + BASE(b) - g(b) + 1
+    const int32_t* jconst;                // [n_r]  4 * (P(a) + h(a))
+    unsigned int* work;
+    unsigned long long* scratch;          // [grid][tile_bins]
+};
+
+__device__ __forceinline__ void red_shared_add(uint32_t addr, uint32_t v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+// One pair: lane-resident j (jx,jy,jz), broadcast k = kv.  Returns the fp32 bin bits twice.
+#define G3_PAIR_BITS(kv, lo, hi)                                          \
+    do {                                                                  \
+        const float ex_ = (kv).x - jx, ey_ = (kv).y - jy, ez_ = (kv).z - jz; \
+        const float t2_ = fmaf(ez_, ez_, fmaf(ey_, ey_, ex_ * ex_));      \
+        const float t_ = sqrt_approx(t2_);                                \
+        lo = __float_as_uint(__fmaf_rd(t_, tp.inv_lo, (kv).w));           \
+        hi = __float_as_uint(__fmaf_rd(t_, tp.inv_hi, (kv).w));           \
+    } while (0)
+
+// Redo one pair exactly (64-bit integers, exact edge table) and move its count if the fp32 bin
+// was wrong.  Called only for pairs whose two fp32 bins differ.
+__device__ __noinline__ void fix_pair(float4 kv, float jx, float jy, float jz, uint32_t lo,
+                                      uint32_t Jj, const unsigned long long* __restrict__ T_t,
+                                      int32_t n_t) {
+    const unsigned long long t2 = exact_d2(kv.x - jx, kv.y - jy, kv.z - jz);
+    const int32_t c_exact = bin_search(T_t, n_t, t2);
+    const int32_t kk1 = (int32_t)(kv.w - kMagic);                 // BASE(b) - g(b) + 1, exact
+    const int32_t c_fast = (int32_t)(lo - kMagicBits) - kk1;
+    if (c_exact != c_fast) {
+        const uint32_t addr = Jj + (lo << 2);
+        red_shared_add(addr, 0xFFFFFFFFu);
+        red_shared_add(addr + 4u * (uint32_t)(c_exact - c_fast), 1u);
+    }
+}
+
+template <int kWarps>
+__global__ void __launch_bounds__(kWarps * 32, 1)
+tiled_triplet_kernel(TriParams tp) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* tile = reinterpret_cast<uint32_t*>(smem_raw);
+    const size_t tile_bytes = ((size_t)tp.tile_bins * 4 + 15) & ~size_t(15);
+    float4* win_all = reinterpret_cast<float4*>(smem_raw + tile_bytes);
+    float* tab_addend = reinterpret_cast<float*>(win_all + kWarps * 32);
+    int32_t* tab_j = reinterpret_cast<int32_t*>(tab_addend + tp.n_r);
+    __shared__ unsigned int cta_items;
+
+    for (int32_t i = threadIdx.x; i < tp.tile_bins; i += blockDim.x) tile[i] = 0;
+    for (int32_t i = threadIdx.x; i < tp.n_r; i += blockDim.x) {
+        tab_addend[i] = tp.addend[i];
+        tab_j[i] = tp.jconst[i];
+    }
+    if (threadIdx.x == 0) cta_items = 0;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    float4* win = win_all + wid * 32;
+    const uint32_t guard = (uint32_t)__cvta_generic_to_shared(tile);      // slot 0
+    // shared-window byte address of slot 0 minus the magic bits (mod 2^32), see file header
+    const uint32_t cbase = guard - (kMagicBits << 2);
+    const long long n_items = (tp.total_centres + kItemCentres - 1) / kItemCentres;
+
+    // work queue: a CTA first takes one of its own `cta_item_cap` tickets, then a global item
+    auto fetch_item = [&]() -> long long {
+        unsigned int it = 0xFFFFFFFFu;
+        if (lane == 0 && atomicAdd(&cta_items, 1u) < tp.cta_item_cap) it = atomicAdd(tp.work, 1u);
+        it = __shfl_sync(0xffffffffu, it, 0);
+        return it < n_items ? (long long)it : -1;
+    };
+
+    long long item = fetch_item();
+    if (item >= 0) {
+        long long item_next = fetch_item();
+        long long c = item * kItemCentres;
+        long long c_end = min(c + (long long)kItemCentres, tp.total_centres);
+        int32_t Kn = tp.nbcount[c];
+        float4 v0n = tp.nbv[c * tp.max_nb + lane], v1n = tp.nbv[c * tp.max_nb + 32 + lane];
+        bool more = true;
+        while (more) {
+            const int32_t K = Kn;
+            const float4 v0 = v0n, v1 = v1n;
+            const float4* __restrict__ lv = tp.nbv + c * tp.max_nb;
+            // ---- advance and prefetch the next centre ------------------------------------------
+            ++c;
+            if (c >= c_end) {
+                if (item_next >= 0) {
+                    c = item_next * kItemCentres;
+                    c_end = min(c + (long long)kItemCentres, tp.total_centres);
+                    item_next = fetch_item();
+                } else more = false;
+            }
+            if (more) {
+                Kn = tp.nbcount[c];
+                v0n = tp.nbv[c * tp.max_nb + lane];
+                v1n = tp.nbv[c * tp.max_nb + 32 + lane];
+            }
+            if (K < 2) continue;
+
+            // ---- all unordered pairs of this centre's K neighbours ------------------------------
+            const int32_t nchunks = (K + 31) >> 5;
+            for (int32_t r = 0; r < nchunks; ++r) {
+                const int32_t jidx = (r << 5) + lane;
+                float4 jraw = r == 0 ? v0 : v1;
+                if (r >= 2 && jidx < K) jraw = lv[jidx];
+                const bool jvalid = jidx < K;
+                const int32_t aj = jvalid ? __float_as_int(jraw.w) : 0;
+                const float jx = jvalid ? jraw.x : 0.f, jy = jvalid ? jraw.y : 0.f, jz = jvalid ? jraw.z : 0.f;
+                const uint32_t Jj = cbase + (uint32_t)tab_j[aj];
+                // prefetch the first rectangular window while the triangle runs
+                float4 nextv = v1;
+                if (r + 1 >= 2 && r + 1 < nchunks && ((r + 1) << 5) + lane < K) nextv = lv[((r + 1) << 5) + lane];
+
+                // ---- triangle: k in the same 32-block as j, k > j --------------------------------
+                __syncwarp();
+                win[lane] = make_float4(jx, jy, jz, tab_addend[aj]);
+                __syncwarp();
+                const int32_t kt = min(32, K - (r << 5));
+                int32_t kk = 1;
+                for (; kk + 4 <= kt; kk += 4) {
+                    const float4 k0 = win[kk], k1 = win[kk + 1], k2 = win[kk + 2], k3 = win[kk + 3];
+                    uint32_t l0, h0, l1, h1, l2, h2, l3, h3;
+                    G3_PAIR_BITS(k0, l0, h0);
+                    G3_PAIR_BITS(k1, l1, h1);
+                    G3_PAIR_BITS(k2, l2, h2);
+                    G3_PAIR_BITS(k3, l3, h3);
+                    const bool p0 = lane < kk, p1 = lane < kk + 1, p2 = lane < kk + 2, p3 = lane < kk + 3;
+                    red_shared_add(p0 ? Jj + (l0 << 2) : guard, 1u);
+                    red_shared_add(p1 ? Jj + (l1 << 2) : guard, 1u);
+                    red_shared_add(p2 ? Jj + (l2 << 2) : guard, 1u);
+                    red_shared_add(p3 ? Jj + (l3 << 2) : guard, 1u);
+                    if (((l0 ^ h0) | (l1 ^ h1) | (l2 ^ h2) | (l3 ^ h3)) != 0u) {
+                        if (p0 && l0 != h0) fix_pair(k0, jx, jy, jz, l0, Jj, tp.T_t, tp.n_t);
+                        if (p1 && l1 != h1) fix_pair(k1, jx, jy, jz, l1, Jj, tp.T_t, tp.n_t);
+                        if (p2 && l2 != h2) fix_pair(k2, jx, jy, jz, l2, Jj, tp.T_t, tp.n_t);
+                        if (p3 && l3 != h3) fix_pair(k3, jx, jy, jz, l3, Jj, tp.T_t, tp.n_t);
+                    }
+                }
+                for (; kk < kt; ++kk) {
+                    const float4 kv = win[kk];
+                    uint32_t lo, hi;
+                    G3_PAIR_BITS(kv, lo, hi);
+                    const bool p = lane < kk;
+                    red_shared_add(p ? Jj + (lo << 2) : guard, 1u);
+                    if (p && lo != hi) fix_pair(kv, jx, jy, jz, lo, Jj, tp.T_t, tp.n_t);
+                }
+                // ---- rectangles: k in later 32-blocks, every lane holds a valid j -----------------
+                for (int32_t q = r + 1; q < nchunks; ++q) {
+                    const bool kvalid = (q << 5) + lane < K;
+                    const int32_t ak = kvalid ? __float_as_int(nextv.w) : 0;
+                    __syncwarp();
+                    win[lane] = make_float4(nextv.x, nextv.y, nextv.z, tab_addend[ak]);
+                    __syncwarp();
+                    if (q + 1 < nchunks && ((q + 1) << 5) + lane < K) nextv = lv[((q + 1) << 5) + lane];
+                    const int32_t kc = min(32, K - (q << 5));
+                    int32_t kq = 0;
+                    for (; kq + 4 <= kc; kq += 4) {
+                        const float4 k0 = win[kq], k1 = win[kq + 1], k2 = win[kq + 2], k3 = win[kq + 3];
+                        uint32_t l0, h0, l1, h1, l2, h2, l3, h3;
+                        G3_PAIR_BITS(k0, l0, h0);
+                        G3_PAIR_BITS(k1, l1, h1);
+                        G3_PAIR_BITS(k2, l2, h2);
+                        G3_PAIR_BITS(k3, l3, h3);
+                        red_shared_add(Jj + (l0 << 2), 1u);
+                        red_shared_add(Jj + (l1 << 2), 1u);
+                        red_shared_add(Jj + (l2 << 2), 1u);
+                        red_shared_add(Jj + (l3 << 2), 1u);
+                        if (((l0 ^ h0) | (l1 ^ h1) | (l2 ^ h2) | (l3 ^ h3)) != 0u) {
+                            if (l0 != h0) fix_pair(k0, jx, jy, jz, l0, Jj, tp.T_t, tp.n_t);
+                            if (l1 != h1) fix_pair(k1, jx, jy, jz, l1, Jj, tp.T_t, tp.n_t);
+                            if (l2 != h2) fix_pair(k2, jx, jy, jz, l2, Jj, tp.T_t, tp.n_t);
+                            if (l3 != h3) fix_pair(k3, jx, jy, jz, l3, Jj, tp.T_t, tp.n_t);
+                        }
+                    }
+                    for (; kq < kc; ++kq) {
+                        const float4 kv = win[kq];
+                        uint32_t lo, hi;
+                        G3_PAIR_BITS(kv, lo, hi);
+                        red_shared_add(Jj + (lo << 2), 1u);
+                        if (lo != hi) fix_pair(kv, jx, jy, jz, lo, Jj, tp.T_t, tp.n_t);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    unsigned long long* out = tp.scratch + (size_t)blockIdx.x * tp.tile_bins;
+    for (int32_t i = 1 + threadIdx.x; i < tp.tile_bins; i += blockDim.x) {
+        const uint32_t v = tile[i];
+        if (v) out[i] += v;
+    }
+}
+
+// Mirror the per-CTA partial tiles into the uint64 histogram (step a5) and clear them.
+// One thread per slot; each slot maps to a unique (a, b, c), so no atomics are needed.
+__global__ void __launch_bounds__(256)
+merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restrict__ slot_map,
+             int32_t tile_bins, int32_t grid, int32_t n_r, int32_t n_t,
+             unsigned long long* __restrict__ counts, unsigned long long* __restrict__ stats) {
+    const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= tile_bins) return;
+    unsigned long long v = 0;
+    for (int32_t gidx = 0; gidx < grid; ++gidx) {
+        unsigned long long* p = scratch + (size_t)gidx * tile_bins + i;
+        const unsigned long long x = *p;
+        if (x) { v += x; *p = 0; }
+    }
+    if (v == 0) return;
+    const uint32_t m = slot_map[i];
+    if (m == 0xFFFFFFFFu) { atomicAdd(stats + 3, v); return; }      // must never happen
+    const int32_t a = (int32_t)(m >> 21), b = (int32_t)((m >> 11) & 1023), c = (int32_t)(m & 2047);
+    if (c >= n_t) { atomicAdd(stats + 1, 2ull * v); return; }       // beyond 2 r_max: overflow
+    if (a == b) counts[((size_t)a * n_r + a) * n_t + c] += 2ull * v;
+    else {
+        counts[((size_t)a * n_r + b) * n_t + c] += v;
+        counts[((size_t)b * n_r + a) * n_t + c] += v;
+    }
+}
+
+inline size_t tri_smem_bytes(int64_t tile_bins, int warps, int32_t n_r) {
+    return (((size_t)tile_bins * 4 + 15) & ~size_t(15)) + (size_t)warps * 32 * 16 + (size_t)n_r * 8;
+}
+
+}  // namespace g3
