@@ -74,27 +74,28 @@ __device__ __noinline__ void fix_pair(float4 kv, float jx, float jy, float jz, u
     }
 }
 
-// The j side of a pair as a lane holds it: vector and tile byte offset of its shell row.
+// The j side of a pair: vector and the tile byte offset of its shell row.
 struct JSide {
     float x, y, z;
     uint32_t J;
 };
 
-__device__ __forceinline__ JSide shfl_jside(const JSide& v, int src) {
+__device__ __forceinline__ JSide load_jside(const float4* __restrict__ win, const uint32_t* __restrict__ winJ, int idx) {
+    const float4 v = win[idx];
     JSide r;
-    r.x = __shfl_sync(0xffffffffu, v.x, src);
-    r.y = __shfl_sync(0xffffffffu, v.y, src);
-    r.z = __shfl_sync(0xffffffffu, v.z, src);
-    r.J = __shfl_sync(0xffffffffu, v.J, src);
+    r.x = v.x; r.y = v.y; r.z = v.z; r.J = winJ[idx];
     return r;
 }
 
 // Four independent pairs (j0,k0) .. (j3,k3) of this lane.  pN = the lane really has pair N; a
 // lane without one adds to the guard slot, so every shared atomic is issued by the full warp.
+// kPred = false: all four exist on every lane (the predicates are ignored).
+template <bool kPred>
 __device__ __forceinline__ void four_pairs(const TriParams& tp, uint32_t guard,
                                            const float4 k0, const float4 k1, const float4 k2, const float4 k3,
                                            const JSide& j0, const JSide& j1, const JSide& j2, const JSide& j3,
                                            bool p0, bool p1, bool p2, bool p3) {
+    if (!kPred) p0 = p1 = p2 = p3 = true;
     uint32_t l0, h0, l1, h1, l2, h2, l3, h3;
     pair_bits(k0, j0.x, j0.y, j0.z, tp.inv_lo, tp.inv_hi, l0, h0);
     pair_bits(k1, j1.x, j1.y, j1.z, tp.inv_lo, tp.inv_hi, l1, h1);
@@ -112,46 +113,72 @@ __device__ __forceinline__ void four_pairs(const TriParams& tp, uint32_t guard,
     }
 }
 
-// All unordered pairs inside one 32-block of a neighbour list (entries 0..kt-1 valid, staged in
-// `win`; `own` = this lane's entry).  Recursive halving instead of a lane-vs-broadcast triangle:
-// at level H (16, 8, 4, 2, 1) the block splits into aligned sub-blocks of 2H entries and every
-// pair whose members first differ in bit H is visited: j = lane with bit H cleared (so j < k and
-// a_j <= a_k), k = sub-block base + H + m, with even m taken by the lane whose bit H is clear
-// and odd m by its partner lane ^ H.  A full block costs 8 + 4 + 2 + 1 + 1 = 16 warp iterations
-// for its 496 pairs (97 % of the lane slots used) instead of 31 (50 %).
+// All unordered pairs inside one 32-block of a neighbour list whose entries 0..kt-1 are valid
+// (16 < kt <= 32) and staged in `win` (vectors + addends) and `winJ` (row offsets).
+// Recursive halving: at level H (16, 8, 4, 2, 1) the block splits into aligned sub-blocks of 2H
+// entries and every pair whose members first differ in bit H is visited, j from the lower half
+// (so j < k and a_j <= a_k), k from the upper half.  Each level is an H x H rectangle per
+// sub-block; levels 16, 8 and 4 are register-tiled 2 j x n k per lane, so one broadcast load of
+// a k entry serves two pairs (the shared-memory data pipe, not the issue slots, binds this
+// kernel: DESIGN.md section 5).  A full block takes 16 pair slots per lane for its 496 pairs
+// (97 % of the lane slots used); the lane-vs-broadcast triangle it replaces took 31 (50 %).
 template <bool kFull>
-__device__ __forceinline__ void triangle(const TriParams& tp, const float4* __restrict__ win,
-                                         uint32_t guard, int lane, int32_t kt, const JSide& own) {
-    if (kFull || kt > 16) {                                   // H = 16: k = 16.., two groups of four
-        const JSide j = shfl_jside(own, lane & ~16);
-        const int32_t k0 = 16 + ((lane >> 4) & 1);
-        const float4* kp = win + k0;
-        const int32_t lim = kt - k0;                          // pair `it` exists iff 2 * it < lim
-        four_pairs(tp, guard, kp[0], kp[2], kp[4], kp[6], j, j, j, j,
-                   kFull || 0 < lim, kFull || 2 < lim, kFull || 4 < lim, kFull || 6 < lim);
-        if (kFull || kt > 24)
-            four_pairs(tp, guard, kp[8], kp[10], kp[12], kp[14], j, j, j, j,
-                       kFull || 8 < lim, kFull || 10 < lim, kFull || 12 < lim, kFull || 14 < lim);
+__device__ __forceinline__ void triangle32(const TriParams& tp, const float4* __restrict__ win,
+                                           const uint32_t* __restrict__ winJ, uint32_t guard,
+                                           int lane, int32_t kt, const JSide& own) {
+    {   // H = 16: j = {g, g + 8}, k = 16 + kg + 4 it, it = 0..3
+        const int g = lane & 7, kidx = 16 + (lane >> 3);
+        const JSide ja = load_jside(win, winJ, g), jb = load_jside(win, winJ, g + 8);
+        {
+            const float4 k0 = win[kidx], k1 = win[kidx + 4];
+            four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
+                               kidx < kt, kidx + 4 < kt, kidx < kt, kidx + 4 < kt);
+        }
+        if (kFull || kt > 24) {
+            const float4 k0 = win[kidx + 8], k1 = win[kidx + 12];
+            four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
+                               kidx + 8 < kt, kidx + 12 < kt, kidx + 8 < kt, kidx + 12 < kt);
+        }
     }
-    if (kFull || kt > 8) {                                    // H = 8
-        const JSide j = shfl_jside(own, lane & ~8);
-        const int32_t k0 = (lane & ~15) + 8 + ((lane >> 3) & 1);
-        const float4* kp = win + k0;
-        const int32_t lim = kt - k0;
-        four_pairs(tp, guard, kp[0], kp[2], kp[4], kp[6], j, j, j, j,
-                   kFull || 0 < lim, kFull || 2 < lim, kFull || 4 < lim, kFull || 6 < lim);
+    {   // H = 8, two sub-blocks: j = {b + g, b + g + 4}, k = b + 8 + kg + 4 it, it = 0..1
+        const int b = lane & 16, g = lane & 3, kidx = b + 8 + ((lane >> 2) & 3);
+        const JSide ja = load_jside(win, winJ, b + g), jb = load_jside(win, winJ, b + g + 4);
+        const float4 k0 = win[kidx], k1 = win[kidx + 4];
+        four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
+                           kidx < kt, kidx + 4 < kt, kidx < kt, kidx + 4 < kt);
     }
-    {                                                         // H = 4 (two pairs), 2 and 1 (one each)
-        const JSide j4 = shfl_jside(own, lane & ~4);
-        const JSide j2 = shfl_jside(own, lane & ~2);
-        const JSide j1 = shfl_jside(own, lane & ~1);
-        const int32_t k4 = (lane & ~7) + 4 + ((lane >> 2) & 1);
-        const int32_t k2 = (lane & ~3) + 2 + ((lane >> 1) & 1);
-        const int32_t k1 = lane | 1;
-        const bool even = (lane & 1) == 0;
-        four_pairs(tp, guard, win[k4], win[k4 + 2], win[k2], win[k1], j4, j4, j2, j1,
-                   kFull || k4 < kt, kFull || k4 + 2 < kt, kFull || k2 < kt, even && (kFull || k1 < kt));
+    {   // H = 4 (j = {b + g, b + g + 2}, k = b + 4 + kg), H = 2 and H = 1 (one pair each)
+        const int b8 = lane & 24, g = lane & 1, k4 = b8 + 4 + ((lane >> 1) & 3);
+        const JSide ja = load_jside(win, winJ, b8 + g), jb = load_jside(win, winJ, b8 + g + 2);
+        const int b4 = lane & 28, k2 = b4 + 2 + ((lane >> 1) & 1);
+        const JSide jc = load_jside(win, winJ, b4 + g);
+        const int k1 = lane | 1;
+        const float4 kA = win[k4], kB = win[k2], kC = win[k1];
+        four_pairs<true>(tp, guard, kA, kA, kB, kC, ja, jb, jc, own,
+                         kFull || k4 < kt, kFull || k4 < kt, kFull || k2 < kt, g == 0 && (kFull || k1 < kt));
     }
+}
+
+// Same for a block with 2 <= kt <= 16 valid entries: the 8 x 8, 4 x 4, 2 x 2 and 1 x 1
+// rectangles are spread over all 32 lanes, four pair slots per lane for up to 120 pairs.
+__device__ __forceinline__ void triangle16(const TriParams& tp, const float4* __restrict__ win,
+                                           const uint32_t* __restrict__ winJ, uint32_t guard,
+                                           int lane, int32_t kt) {
+    // H = 8: j = lane & 7, k = 8 + kg + 4 it (it = 0..1)
+    const int kidx = 8 + (lane >> 3);
+    const JSide ja = load_jside(win, winJ, lane & 7);
+    // H = 4, two sub-blocks: j = b + (lane & 3), k = b + 4 + kg
+    const int b = (lane >> 4) << 3, k4 = b + 4 + ((lane >> 2) & 3);
+    const JSide jb = load_jside(win, winJ, b + (lane & 3));
+    // H = 2 on lanes 0..15 (four sub-blocks), H = 1 on lanes 16..23 (eight pairs)
+    const bool low = lane < 16;
+    const int b4 = (lane >> 2) << 2;
+    const int jl = low ? b4 + (lane & 1) : 2 * (lane & 7);
+    const int kl = low ? b4 + 2 + ((lane >> 1) & 1) : 2 * (lane & 7) + 1;
+    const JSide jc = load_jside(win, winJ, jl);
+    const float4 k0 = win[kidx], k1 = win[kidx + 4], kB = win[k4], kC = win[kl];
+    four_pairs<true>(tp, guard, k0, k1, kB, kC, ja, ja, jb, jc,
+                     kidx < kt, kidx + 4 < kt, k4 < kt, lane < 24 && kl < kt);
 }
 
 template <int kWarps>
@@ -160,8 +187,9 @@ tiled_triplet_kernel(TriParams tp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t* tile = reinterpret_cast<uint32_t*>(smem_raw);
     const size_t tile_bytes = ((size_t)tp.tile_bins * 4 + 15) & ~size_t(15);
-    float4* win_all = reinterpret_cast<float4*>(smem_raw + tile_bytes);
-    float* tab_addend = reinterpret_cast<float*>(win_all + kWarps * 32);
+    float4* win_all = reinterpret_cast<float4*>(smem_raw + tile_bytes);       // [warp][2][32]
+    uint32_t* winJ_all = reinterpret_cast<uint32_t*>(win_all + kWarps * 64);  // [warp][32]
+    float* tab_addend = reinterpret_cast<float*>(winJ_all + kWarps * 32);
     int32_t* tab_j = reinterpret_cast<int32_t*>(tab_addend + tp.n_r);
     __shared__ unsigned int cta_items;
 
@@ -174,7 +202,9 @@ tiled_triplet_kernel(TriParams tp) {
     __syncthreads();
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float4* win = win_all + wid * 32;
+    float4* winA = win_all + wid * 64;          // the 32-block the j side comes from
+    float4* winB = winA + 32;                   // the later 32-block the k side comes from
+    uint32_t* winJ = winJ_all + wid * 32;       // tile row offsets of winA's entries
     const uint32_t guard = (uint32_t)__cvta_generic_to_shared(tile);      // slot 0
     // shared-window byte address of slot 0 minus the magic bits (mod 2^32), see file header
     const uint32_t cbase = guard - (kMagicBits << 2);
@@ -233,28 +263,36 @@ tiled_triplet_kernel(TriParams tp) {
 
                 // ---- triangle: both members in this 32-block -------------------------------------
                 __syncwarp();
-                win[lane] = make_float4(own.x, own.y, own.z, tab_addend[aj]);
+                winA[lane] = make_float4(own.x, own.y, own.z, tab_addend[aj]);
+                winJ[lane] = own.J;
                 __syncwarp();
                 const int32_t kt = min(32, K - (r << 5));
-                if (kt == 32) triangle<true>(tp, win, guard, lane, kt, own);
-                else triangle<false>(tp, win, guard, lane, kt, own);
+                if (kt == 32) triangle32<true>(tp, winA, winJ, guard, lane, kt, own);
+                else if (kt > 16) triangle32<false>(tp, winA, winJ, guard, lane, kt, own);
+                else if (kt >= 2) triangle16(tp, winA, winJ, guard, lane, kt);
+                if (r + 1 == nchunks) break;
 
-                // ---- rectangles: k in later 32-blocks, every lane holds a valid j -----------------
+                // ---- rectangles: k in later 32-blocks; this block is full, 2 j x 2 k per lane ----
+                const int kg = lane >> 4;
+                const JSide ja = load_jside(winA, winJ, lane & 15), jb = load_jside(winA, winJ, (lane & 15) + 16);
                 for (int32_t q = r + 1; q < nchunks; ++q) {
                     const bool kvalid = (q << 5) + lane < K;
                     const int32_t ak = kvalid ? __float_as_int(nextv.w) : 0;
                     __syncwarp();
-                    win[lane] = make_float4(nextv.x, nextv.y, nextv.z, tab_addend[ak]);
+                    winB[lane] = make_float4(kvalid ? nextv.x : 0.f, kvalid ? nextv.y : 0.f,
+                                             kvalid ? nextv.z : 0.f, tab_addend[ak]);
                     __syncwarp();
                     if (q + 1 < nchunks && ((q + 1) << 5) + lane < K) nextv = lv[((q + 1) << 5) + lane];
                     const int32_t kc = min(32, K - (q << 5));
-                    int32_t kq = 0;
-                    for (; kq + 4 <= kc; kq += 4)
-                        four_pairs(tp, guard, win[kq], win[kq + 1], win[kq + 2], win[kq + 3],
-                                   own, own, own, own, true, true, true, true);
-                    if (kq < kc)                                    // 1..3 left: predicate, do not branch
-                        four_pairs(tp, guard, win[kq], win[min(kq + 1, 31)], win[min(kq + 2, 31)], win[0],
-                                   own, own, own, own, true, kq + 1 < kc, kq + 2 < kc, false);
+                    for (int32_t k0i = 0; k0i < kc; k0i += 4) {     // k = k0i + kg and k0i + kg + 2
+                        const int32_t kidx = k0i + kg;
+                        const float4 k0 = winB[kidx], k1 = winB[kidx + 2];
+                        if (k0i + 4 <= kc)
+                            four_pairs<false>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, true, true, true, true);
+                        else
+                            four_pairs<true>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb,
+                                             kidx < kc, kidx < kc, kidx + 2 < kc, kidx + 2 < kc);
+                    }
                 }
             }
         }
@@ -294,7 +332,7 @@ merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restric
 }
 
 inline size_t tri_smem_bytes(int64_t tile_bins, int warps, int32_t n_r) {
-    return (((size_t)tile_bins * 4 + 15) & ~size_t(15)) + (size_t)warps * 32 * 16 + (size_t)n_r * 8;
+    return (((size_t)tile_bins * 4 + 15) & ~size_t(15)) + (size_t)warps * (64 * 16 + 32 * 4) + (size_t)n_r * 8;
 }
 
 }  // namespace g3
