@@ -48,12 +48,19 @@ __device__ __forceinline__ unsigned long long exact_d2(float dx, float dy, float
     return (unsigned long long)(X * X + Y * Y + Z * Z);
 }
 
-// Phase A for 32 candidates: `c` is this lane's candidate (relative coordinates), `in` says
-// whether it is a real candidate other than the centre itself.
+__device__ __forceinline__ void sts128(uint32_t addr, float x, float y, float z, float w) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+
+constexpr float kFarAway = 3.0e18f;            // sentinel coordinate: its d2 is finite and beyond any cut-off
+
+// Phase A for 32 candidates: `c` is this lane's candidate, `skip` = it is the centre itself.
+// Accepted candidates are ballot-compacted into the warp's scratch list (shared address
+// `scratch_s`, 16 B per entry) as (dx, dy, dz, d2).
 template <bool kWrap>
-__device__ __forceinline__ void nb_test(float4 c, bool in, float px, float py, float pz,
-                                        float cut_hi, int lane, int32_t max_nb, float4* scratch,
-                                        int32_t& count) {
+__device__ __forceinline__ void nb_test(const float4 c, bool skip, float px, float py, float pz,
+                                        float cut_hi, uint32_t lt_mask, int32_t max_nb,
+                                        uint32_t scratch_s, int32_t& count) {
     float dx = c.x - px, dy = c.y - py, dz = c.z - pz;
     if (kWrap) {
         dx += dx < -524288.f ? 1048576.f : 0.f; dx -= dx >= 524288.f ? 1048576.f : 0.f;
@@ -61,10 +68,10 @@ __device__ __forceinline__ void nb_test(float4 c, bool in, float px, float py, f
         dz += dz < -524288.f ? 1048576.f : 0.f; dz -= dz >= 524288.f ? 1048576.f : 0.f;
     }
     const float d2f = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const bool acc = in && d2f < cut_hi;
+    const bool acc = d2f < cut_hi && !skip;
     const unsigned mask = __ballot_sync(0xffffffffu, acc);
-    const int32_t pos = count + __popc(mask & ((1u << lane) - 1u));
-    if (acc && pos < max_nb) scratch[pos] = make_float4(dx, dy, dz, d2f);
+    const int32_t pos = count + __popc(mask & lt_mask);
+    if (acc && pos < max_nb) sts128(scratch_s + ((uint32_t)pos << 4), dx, dy, dz, d2f);
     count += __popc(mask);
 }
 
@@ -108,7 +115,8 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
     const int32_t c_begin = cell_range[0], c_end = cell_range[1];
     if (c_begin == c_end) return;                         // empty cell: no centres
     const int32_t n_stage = range_prefix[n_ranges];
-    const bool staged = n_stage <= np.stage_cap;
+    const int32_t n_pad = (n_stage + 31) & ~31;           // stage padded with far-away sentinels
+    const bool staged = n_pad <= np.stage_cap;
     int32_t ox = 0, oy = 0, oz = 0;
     if (!kWrap) {
         const int32_t cz = cell % fb.ncell, cy = (cell / fb.ncell) % fb.ncell, cx = cell / (fb.ncell * fb.ncell);
@@ -121,19 +129,24 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
         return make_float4((float)wrap_component(c.x - ox), (float)wrap_component(c.y - oy),
                            (float)wrap_component(c.z - oz), 0.f);
     };
-    if (staged) {
-        for (int32_t d = threadIdx.x; d < n_stage; d += blockDim.x) {
-            int32_t r = 0;
-            while (d >= range_prefix[r + 1]) ++r;
-            stage[d] = relative(sorted[range_begin[r] + (d - range_prefix[r])]);
+    if (staged) {                                         // a warp per range: straight copies
+        for (int32_t r = wid; r < n_ranges; r += kNbWarps) {
+            const int32_t b = range_begin[r], dst = range_prefix[r], len = range_prefix[r + 1] - dst;
+            for (int32_t i = lane; i < len; i += 32) stage[dst + i] = relative(sorted[b + i]);
         }
+        for (int32_t i = n_stage + threadIdx.x; i < n_pad; i += blockDim.x)
+            stage[i] = make_float4(kFarAway, 0.f, 0.f, 0.f);
         __syncthreads();
     }
 
     // ---- one warp per centre -------------------------------------------------------------------
     float4* scratch = scratch_all + (size_t)wid * np.max_nb;
-    int32_t* hist = hist_all + (size_t)wid * (np.n_r + 1);
+    int32_t* hist = hist_all + (size_t)wid * ((np.n_r + 3) & ~1);   // even stride: 8-byte aligned pairs
+    const uint32_t scratch_s = (uint32_t)__cvta_generic_to_shared(scratch);
+    const uint32_t lt_mask = (1u << lane) - 1u;
     const int32_t own_base = own_base_s;
+    const int32_t max_nb = np.max_nb, n_r = np.n_r;
+    const float cut_hi = np.cut_hi;
     // degenerate grid: the centres are split over blockIdx.y in slices of 64
     const int32_t s_lo = kWrap ? min(c_end, (int32_t)blockIdx.y * 64) : c_begin;
     const int32_t s_hi = kWrap ? min(c_end, (int32_t)(blockIdx.y + 1) * 64) : c_end;
@@ -144,12 +157,13 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
         if (staged) {
             const int32_t own = own_base + (s - c_begin);
             const float4 p = stage[own];
-            for (int32_t q0 = 0; q0 < n_stage; q0 += 32) {
-                const int32_t q = q0 + lane;
-                const bool in = q < n_stage && q != own;
-                const float4 c = in ? stage[q] : p;
-                nb_test<kWrap>(c, in, p.x, p.y, p.z, np.cut_hi, lane, np.max_nb, scratch, count);
-            }
+            const int32_t own_q0 = own & ~31;
+            const bool own_lane = lane == (own & 31);
+            const float4* __restrict__ sp = stage + lane;
+#pragma unroll 2
+            for (int32_t q0 = 0; q0 < n_pad; q0 += 32)
+                nb_test<kWrap>(sp[q0], own_lane && q0 == own_q0, p.x, p.y, p.z, cut_hi, lt_mask, max_nb,
+                               scratch_s, count);
         } else {                                           // crowded neighbourhood: read from global
             const float4 p = relative(sorted[s]);
             for (int32_t r = 0; r < n_ranges; ++r) {
@@ -158,12 +172,12 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
                     const int32_t q = q0 + lane;
                     const bool in = q < e && q != s;
                     const float4 c = in ? relative(sorted[q]) : p;
-                    nb_test<kWrap>(c, in, p.x, p.y, p.z, np.cut_hi, lane, np.max_nb, scratch, count);
+                    nb_test<kWrap>(c, !in, p.x, p.y, p.z, cut_hi, lt_mask, max_nb, scratch_s, count);
                 }
             }
         }
-        if (count > np.max_nb) { my_cap += 1; count = np.max_nb; }
-        for (int32_t i = lane; i <= np.n_r; i += 32) hist[i] = 0;
+        if (count > max_nb) { my_cap += 1; count = max_nb; }
+        for (int32_t i = lane; i < n_r + 2; i += 32) hist[i] = 0;
         __syncwarp();
 
         // phase B: exact acceptance near the cut-off, shell, rank inside the shell
@@ -176,7 +190,7 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
                 have_exact = true;
                 keep = d2 < np.cut2;
             }
-            int32_t a = np.n_r;                            // n_r = rejected
+            int32_t a = n_r;                               // n_r = rejected
             if (keep) {
                 const float t = sqrt_approx(v.w);
                 const uint32_t lo = __float_as_uint(__fmaf_rd(t, np.inv_w_lo, kMagic));
@@ -184,7 +198,7 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
                 if (lo == hi) a = (int32_t)(lo - kMagicBits);
                 else {
                     if (!have_exact) d2 = exact_d2(v.x, v.y, v.z);
-                    a = bin_search(np.T_r, np.n_r, d2);
+                    a = bin_search(np.T_r, n_r, d2);
                 }
             }
             const int32_t rank = atomicAdd(hist + a, 1);
@@ -192,29 +206,35 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
         }
         __syncwarp();
 
-        // phase C: exclusive scan of the shell counts, scatter in shell order
+        // phase C: exclusive scan of the shell counts (two shells per lane), scatter in shell order
         int32_t carry = 0;
-        for (int32_t i0 = 0; i0 < np.n_r; i0 += 32) {
-            const int32_t i = i0 + lane;
-            const int32_t v = i < np.n_r ? hist[i] : 0;
+        for (int32_t i0 = 0; i0 < n_r; i0 += 64) {
+            const int32_t i = i0 + 2 * lane;
+            int2 hv = make_int2(0, 0);                     // hist has >= n_r + 2 entries, i is even
+            if (i < n_r) hv = *reinterpret_cast<const int2*>(hist + i);
+            const int32_t v0 = i < n_r ? hv.x : 0, v1 = i + 1 < n_r ? hv.y : 0;
+            const int32_t v = v0 + v1;
             int32_t incl = v;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
                 const int32_t t = __shfl_up_sync(0xffffffffu, incl, d);
                 if (lane >= d) incl += t;
             }
-            if (i < np.n_r) hist[i] = carry + incl - v;
-            carry += __shfl_sync(0xffffffffu, incl, 31);
+            const int32_t total = __shfl_sync(0xffffffffu, incl, 31);
+            __syncwarp();
+            if (i < n_r) hist[i] = carry + incl - v;
+            if (i + 1 < n_r) hist[i + 1] = carry + incl - v1;
+            carry += total;
         }
         __syncwarp();
         const int32_t kept = carry;
         my_pairs += (unsigned long long)kept * (unsigned long long)(kept > 0 ? kept - 1 : 0);
-        const long long gbase = ((long long)f * fb.n + s) * np.max_nb;
+        float4* __restrict__ dst = np.nbv + ((long long)f * fb.n + s) * max_nb;
         for (int32_t e = lane; e < count; e += 32) {
             const float4 v = scratch[e];
             const int32_t packed = __float_as_int(v.w);
             const int32_t a = packed & 1023, rank = packed >> 10;
-            if (a < np.n_r) np.nbv[gbase + hist[a] + rank] = make_float4(v.x, v.y, v.z, __int_as_float(a));
+            if (a < n_r) dst[hist[a] + rank] = make_float4(v.x, v.y, v.z, __int_as_float(a));
         }
         if (lane == 0) np.nbcount[(long long)f * fb.n + s] = kept;
         __syncwarp();
@@ -226,7 +246,7 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
 }
 
 inline size_t nb_smem_bytes(int32_t stage_cap, int32_t max_nb, int32_t n_r) {
-    return (size_t)stage_cap * 16 + (size_t)kNbWarps * max_nb * 16 + (size_t)kNbWarps * (n_r + 1) * 4;
+    return (size_t)stage_cap * 16 + (size_t)kNbWarps * max_nb * 16 + (size_t)kNbWarps * ((n_r + 3) & ~1) * 4;
 }
 
 }  // namespace g3
