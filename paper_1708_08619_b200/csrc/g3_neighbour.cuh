@@ -32,6 +32,7 @@ struct NbParams {
     unsigned long long cut2;
     float inv_w_lo, inv_w_hi;             // (1/w)(1 -+ 2^-20), w = shell width in grid units
     const unsigned long long* T_r;
+    const int4* cell_origin;              // [ncell3] grid coordinates of the cell centres
     float4* nbv;                          // [frames][n][max_nb] (dx, dy, dz, shell as int bits)
     int32_t* nbcount;                     // [frames][n]
     unsigned long long* stats;
@@ -88,7 +89,8 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
     __shared__ int32_t own_base_s, cell_range[2];
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int32_t f = blockIdx.x / fb.ncell3, cell = blockIdx.x - f * fb.ncell3;
+    // grid: x = cell (or slice of 64 centres when the cell grid is degenerate), y = frame
+    const int32_t f = blockIdx.y, cell = kWrap ? 0 : blockIdx.x;
     const int4* __restrict__ sorted = fb.sorted + (long long)f * fb.n;
     const int32_t* __restrict__ start = fb.cell_start + (long long)f * (fb.ncell3 + 1);
 
@@ -119,10 +121,8 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
     const bool staged = n_pad <= np.stage_cap;
     int32_t ox = 0, oy = 0, oz = 0;
     if (!kWrap) {
-        const int32_t cz = cell % fb.ncell, cy = (cell / fb.ncell) % fb.ncell, cx = cell / (fb.ncell * fb.ncell);
-        ox = (int32_t)(((long long)(2 * cx + 1) << (kGridBits - 1)) / fb.ncell);   // cell centre
-        oy = (int32_t)(((long long)(2 * cy + 1) << (kGridBits - 1)) / fb.ncell);
-        oz = (int32_t)(((long long)(2 * cz + 1) << (kGridBits - 1)) / fb.ncell);
+        const int4 o = __ldg(np.cell_origin + cell);
+        ox = o.x; oy = o.y; oz = o.z;
     }
     auto relative = [&](int4 c) {
         if (kWrap) return make_float4((float)c.x, (float)c.y, (float)c.z, 0.f);
@@ -147,9 +147,9 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
     const int32_t own_base = own_base_s;
     const int32_t max_nb = np.max_nb, n_r = np.n_r;
     const float cut_hi = np.cut_hi;
-    // degenerate grid: the centres are split over blockIdx.y in slices of 64
-    const int32_t s_lo = kWrap ? min(c_end, (int32_t)blockIdx.y * 64) : c_begin;
-    const int32_t s_hi = kWrap ? min(c_end, (int32_t)(blockIdx.y + 1) * 64) : c_end;
+    // degenerate grid: the centres are split over blockIdx.x in slices of 64
+    const int32_t s_lo = kWrap ? min(c_end, (int32_t)blockIdx.x * 64) : c_begin;
+    const int32_t s_hi = kWrap ? min(c_end, (int32_t)(blockIdx.x + 1) * 64) : c_end;
     unsigned long long my_pairs = 0, my_cap = 0;
     for (int32_t s = s_lo + wid; s < s_hi; s += kNbWarps) {
         int32_t count = 0;

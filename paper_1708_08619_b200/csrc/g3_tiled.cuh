@@ -35,6 +35,7 @@ struct TiledState {
     float4* d_nbv = nullptr;                   // [batch][n][max_nb] (dx, dy, dz, shell)
     int32_t* d_nbcount = nullptr;              // [batch][n]
     unsigned int* d_work = nullptr;            // work-queue counter
+    int4* d_cell_origin = nullptr;             // [ncell3] cell centres on the grid
     // launch configuration
     int tri_warps = 16;
     int grid = 0;
@@ -126,7 +127,7 @@ inline void tiled_free(g3_plan* p) {
     TiledState* ts = p->tiled;
     if (!ts) return;
     cudaFree(ts->d_addend); cudaFree(ts->d_jconst); cudaFree(ts->d_slot_map); cudaFree(ts->d_scratch);
-    cudaFree(ts->d_nbv); cudaFree(ts->d_nbcount); cudaFree(ts->d_work);
+    cudaFree(ts->d_nbv); cudaFree(ts->d_nbcount); cudaFree(ts->d_work); cudaFree(ts->d_cell_origin);
     delete ts;
     p->tiled = nullptr;
 }
@@ -202,6 +203,19 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMalloc(&ts->d_nbv, sizeof(float4) * (per_frame_entries * B + 64)));   // +64: prefetch overrun
     G3T_CUDA(cudaMalloc(&ts->d_nbcount, sizeof(int32_t) * (size_t)p->n * B));
     G3T_CUDA(cudaMalloc(&ts->d_work, sizeof(unsigned int)));
+    {
+        const int32_t nc = p->ncell;
+        std::vector<int4> origin((size_t)nc * nc * nc);
+        for (int32_t cx = 0; cx < nc; ++cx)
+            for (int32_t cy = 0; cy < nc; ++cy)
+                for (int32_t cz = 0; cz < nc; ++cz)
+                    origin[((size_t)cx * nc + cy) * nc + cz] =
+                        make_int4((int32_t)(((int64_t)(2 * cx + 1) << (kGridBits - 1)) / nc),
+                                  (int32_t)(((int64_t)(2 * cy + 1) << (kGridBits - 1)) / nc),
+                                  (int32_t)(((int64_t)(2 * cz + 1) << (kGridBits - 1)) / nc), 0);
+        G3T_CUDA(cudaMalloc(&ts->d_cell_origin, sizeof(int4) * origin.size()));
+        G3T_CUDA(cudaMemcpy(ts->d_cell_origin, origin.data(), sizeof(int4) * origin.size(), cudaMemcpyHostToDevice));
+    }
     G3T_CUDA(cudaMemcpy(ts->d_addend, addend.data(), sizeof(float) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_jconst, jconst.data(), sizeof(int32_t) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_slot_map, slot_map.data(), sizeof(uint32_t) * ts->tile_bins, cudaMemcpyHostToDevice));
@@ -242,6 +256,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     np.inv_w_lo = (float)((1.0 / w) * (1.0 - eps));
     np.inv_w_hi = (float)((1.0 / w) * (1.0 + eps));
     np.T_r = bs.T_r;
+    np.cell_origin = ts->d_cell_origin;
     np.nbv = ts->d_nbv; np.nbcount = ts->d_nbcount; np.stats = p->d_stats;
     G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -257,10 +272,10 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         G3T_CUDA(cudaEventRecord(ev[0], st));
     }
     if (fb.ncell == 1) {
-        dim3 grid((unsigned)fb.n_frames, (unsigned)((fb.n + 63) / 64));
+        dim3 grid((unsigned)((fb.n + 63) / 64), (unsigned)fb.n_frames);
         neighbour_kernel<true><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
     } else {
-        dim3 grid((unsigned)((long long)fb.n_frames * fb.ncell3), 1);
+        dim3 grid((unsigned)fb.ncell3, (unsigned)fb.n_frames);
         neighbour_kernel<false><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
     }
     if (p->timing) G3T_CUDA(cudaEventRecord(ev[1], st));
