@@ -40,6 +40,10 @@ UNIT = "triplets/s"
 WORKLOAD_INDEX = 4
 ALGO_INSTR_PER_TRIPLET = 12          # fixed algorithmic instruction count
 SM_LANES = 128                       # 4 schedulers x 32 lanes, one warp instruction per cycle each
+# dram__bytes_read.sum + dram__bytes_write.sum of one tiled_triplet_kernel launch (16 frames of
+# config 4) from the ncu --set full capture summarised in profiles/r1_triplet_kernel.md
+NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH = 598.814464e6 + 8.376832e6
+NCU_TRIPLET_FRAMES_PER_LAUNCH = 16
 
 
 def peaks():
@@ -285,7 +289,11 @@ def run_ours(args):
     achieved = trip_per_launch * ALGO_INSTR_PER_TRIPLET / tri_s / 1e12 if tri_s > 0 else 0.0
     roofline = {
         "bound": "alu", "kernel": "tiled_triplet_kernel", "achieved": achieved, "peak": peak_tinstr,
-        "unit": "Tinstr/s", "frac": achieved / peak_tinstr, "traffic": None,
+        "unit": "Tinstr/s", "frac": achieved / peak_tinstr,
+        "traffic": (NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH
+                    if plan.info(g3.G3_INFO_BATCH_FRAMES) == NCU_TRIPLET_FRAMES_PER_LAUNCH and not args.frames
+                    else None),
+        "traffic_unit": "bytes of DRAM traffic per launch (ncu, profiles/r1_triplet_kernel.md)",
         "peak_kind": f"{sm_count} SMs x {SM_LANES} lanes x sm_max_mhz ({pk_kind}); DESIGN.md 6",
         "algorithmic_instr_per_triplet": ALGO_INSTR_PER_TRIPLET,
         "triplets_per_launch": trip_per_launch, "kernel_ms_per_launch": tri_s * 1e3,
