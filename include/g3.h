@@ -98,7 +98,11 @@ typedef enum {
      * sums cover the launches since creation or the last g3_plan_clear_timing.             */
     G3_INFO_TRIPLET_NS = 9,      /* device time of the triplet kernel launches, nanoseconds  */
     G3_INFO_NEIGHBOUR_NS = 10,   /* device time of the neighbour kernel launches             */
-    G3_INFO_TIMED_LAUNCHES = 11  /* launches of EACH of the two kernels covered by the sums  */
+    G3_INFO_TIMED_LAUNCHES = 11, /* launches of EACH of the two kernels covered by the sums
+                                    (a triplet "launch" = all slab passes of one batch)      */
+    G3_INFO_SLABS = 12           /* tiled kernel: slab passes per batch (1 = the reachable bins
+                                    fit one shared-memory tile; G3_INFO_TILE_BINS counts all
+                                    reachable slots, over all slabs)                          */
 } g3_info;
 
 /* Create a plan for frames of `n` particles in a cubic periodic box of edge `box`

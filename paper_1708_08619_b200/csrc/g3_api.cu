@@ -308,6 +308,7 @@ int g3_plan_get_info(const g3_plan* cp, int32_t key, int64_t* value) {
         case G3_INFO_TILE_BINS: *value = p->tile_bins; break;
         case G3_INFO_SM_COUNT: *value = p->sm_count; break;
         case G3_INFO_FRAMES_PENDING: *value = p->pending; break;
+        case G3_INFO_SLABS: *value = p->tiled ? p->tiled->n_slabs : 0; break;
         default: return G3_EINVAL;
     }
     return G3_OK;

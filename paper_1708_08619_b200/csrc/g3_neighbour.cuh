@@ -36,6 +36,10 @@ struct NbParams {
     float4* nbv;                          // [frames][n][max_nb] (dx, dy, dz, shell as int bits)
     int32_t* nbcount;                     // [frames][n]
     unsigned long long* stats;
+    // slab passes of the triplet kernel (n_slabs > 1): list position where each slab's shells start
+    int32_t n_slabs;
+    const int32_t* slab_shell;            // [n_slabs + 1] first shell of each slab; [n_slabs] = n_r
+    int32_t* slabpos;                     // [frames][n][n_slabs + 1]
 };
 
 __device__ __forceinline__ float sqrt_approx(float x) {
@@ -237,6 +241,13 @@ neighbour_kernel(FrameBatch fb, NbParams np) {
             if (a < n_r) dst[hist[a] + rank] = make_float4(v.x, v.y, v.z, __int_as_float(a));
         }
         if (lane == 0) np.nbcount[(long long)f * fb.n + s] = kept;
+        if (np.n_slabs > 1) {                     // hist[a] = list position of the first entry of shell a
+            int32_t* sp = np.slabpos + ((long long)f * fb.n + s) * (np.n_slabs + 1);
+            for (int32_t i = lane; i <= np.n_slabs; i += 32) {
+                const int32_t a = np.slab_shell[i];
+                sp[i] = a < n_r ? hist[a] : kept;
+            }
+        }
         __syncwarp();
     }
     if (lane == 0) {

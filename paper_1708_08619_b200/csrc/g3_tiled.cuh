@@ -44,7 +44,32 @@ struct TiledState {
     uint32_t cta_item_cap = 0;                 // work items one CTA may take per launch
     int64_t max_batch_frames = 1;              // frames per launch the item cap allows
     bool dirty = false;                        // partial tiles hold counts not yet merged
+    // slab passes: when the whole tile does not fit shared memory the outer shell b is split
+    // into n_slabs ranges [slab_shell[s], slab_shell[s+1]); one triplet launch per slab
+    int32_t n_slabs = 1;
+    std::vector<int32_t> slab_shell;           // [n_slabs + 1]
+    int64_t slab_bins_max = 0;                 // slots (incl. 2 guards) of the largest slab
+    int32_t* d_slab_shell = nullptr;
+    int32_t* d_slabpos = nullptr;              // [batch][n][n_slabs + 1]
 };
+
+// Split the outer shell range so that every slab's slots fit `cap_slots`.  False if one
+// column block alone is too large.
+inline bool build_slabs(TiledState& ts, int32_t n_r, int64_t cap_slots) {
+    ts.slab_shell.assign(1, 0);
+    ts.slab_bins_max = 0;
+    int32_t b0 = 0;
+    while (b0 < n_r) {
+        int32_t b1 = b0;
+        while (b1 < n_r && (int64_t)ts.BASE[b1 + 1] - ts.BASE[b0] + 2 <= cap_slots) ++b1;
+        if (b1 == b0) return false;
+        ts.slab_bins_max = std::max<int64_t>(ts.slab_bins_max, (int64_t)ts.BASE[b1] - ts.BASE[b0] + 2);
+        ts.slab_shell.push_back(b1);
+        b0 = b1;
+    }
+    ts.n_slabs = (int32_t)ts.slab_shell.size() - 1;
+    return true;
+}
 
 // ---------------------------------------------------------------------------------------------
 // host: histogram tile layout
@@ -109,15 +134,33 @@ inline int tiled_warps(const g3_plan* p, int64_t tile_bins) {
     return w;
 }
 
+// Slots a tile may hold beside the windows of `warps` warps and the shell tables.
+inline int64_t tiled_cap_slots(const g3_plan* p, int warps) {
+    const int64_t fixed = (int64_t)tri_smem_bytes(0, warps, p->bins.n_r) + 64;   // + static shared
+    return ((int64_t)p->smem_optin - fixed) / 4;
+}
+
+// Layout + slabs for this plan; false if the tiled path cannot serve it.
+inline bool tiled_plan_slabs(const g3_plan* p, TiledState& ts) {
+    build_layout(p, ts);
+    if (ts.tile_bins > (1 << 22)) return false;                    // addend must stay below 2^24
+    if (tri_smem_bytes(ts.tile_bins, 8, p->bins.n_r) <= (size_t)p->smem_optin) {
+        ts.n_slabs = 1;
+        ts.slab_shell = {0, p->bins.n_r};
+        ts.slab_bins_max = ts.tile_bins;
+        return true;
+    }
+    const int warps = p->tri_warps_opt ? p->tri_warps_opt : 24;
+    return build_slabs(ts, p->bins.n_r, tiled_cap_slots(p, warps)) && ts.n_slabs <= 64;
+}
+
 // 2 if the tiled path can serve this plan, else 1 (generic).
 inline int32_t tiled_select(g3_plan* p) {
     if (p->kernel_opt == 1) return 1;
     if (p->bins.n_r > 1022 || p->bins.n_t > 2046) return 1;
     if (p->max_nb > (1 << 16)) return 1;
     TiledState ts;
-    build_layout(p, ts);
-    if (ts.tile_bins > (1 << 22)) return 1;                        // addend must stay below 2^24
-    if (tri_smem_bytes(ts.tile_bins, 8, p->bins.n_r) > (size_t)p->smem_optin) return 1;   // TODO slabs
+    if (!tiled_plan_slabs(p, ts)) return 1;
     if (nb_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r) > (size_t)p->smem_optin) return 1;
     if (p->ncell == 1 && p->n > 8192) return 1;
     return 2;
@@ -128,6 +171,7 @@ inline void tiled_free(g3_plan* p) {
     if (!ts) return;
     cudaFree(ts->d_addend); cudaFree(ts->d_jconst); cudaFree(ts->d_slot_map); cudaFree(ts->d_scratch);
     cudaFree(ts->d_nbv); cudaFree(ts->d_nbcount); cudaFree(ts->d_work); cudaFree(ts->d_cell_origin);
+    cudaFree(ts->d_slab_shell); cudaFree(ts->d_slabpos);
     delete ts;
     p->tiled = nullptr;
 }
@@ -143,9 +187,19 @@ inline void tiled_free(g3_plan* p) {
 
 template <int kWarps>
 inline int tiled_set_attr(size_t smem) {
-    G3T_CUDA(cudaFuncSetAttribute(tiled_triplet_kernel<kWarps>,
+    G3T_CUDA(cudaFuncSetAttribute(tiled_triplet_kernel<kWarps, false>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    G3T_CUDA(cudaFuncSetAttribute(tiled_triplet_kernel<kWarps, true>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     return G3_OK;
+}
+
+template <int kWarps>
+inline void tiled_launch_triplet(const TiledState* ts, const TriParams& tp, cudaStream_t st) {
+    if (ts->n_slabs > 1)
+        tiled_triplet_kernel<kWarps, true><<<ts->grid, kWarps * 32, ts->tri_smem, st>>>(tp);
+    else
+        tiled_triplet_kernel<kWarps, false><<<ts->grid, kWarps * 32, ts->tri_smem, st>>>(tp);
 }
 
 inline int tiled_configure(g3_plan* p) {
@@ -153,7 +207,7 @@ inline int tiled_configure(g3_plan* p) {
     TiledState* ts = new (std::nothrow) TiledState;
     if (!ts) return G3_ENOMEM;
     p->tiled = ts;
-    build_layout(p, *ts);
+    if (!tiled_plan_slabs(p, *ts)) return G3_EINVAL;
     p->tile_bins = ts->tile_bins;
     const int32_t n_r = p->bins.n_r;
 
@@ -167,13 +221,13 @@ inline int tiled_configure(g3_plan* p) {
     ts->max_batch_frames = (int64_t)((long double)ts->grid * ts->cta_item_cap * kItemCentres / (long double)p->n);
     if (ts->max_batch_frames < 1) return G3_EINVAL;
     if (p->batch_frames > ts->max_batch_frames) p->batch_frames = (int32_t)ts->max_batch_frames;
-    // neighbour lists of one batch: keep them below ~4 GiB
+    // neighbour lists of one batch: keep them below ~16 GiB
     const size_t frame_bytes = (size_t)p->n * p->max_nb * sizeof(float4);
-    const int64_t mem_frames = std::max<int64_t>(1, (int64_t)((size_t(4) << 30) / frame_bytes));
+    const int64_t mem_frames = std::max<int64_t>(1, (int64_t)((size_t(16) << 30) / frame_bytes));
     if (p->batch_frames > mem_frames) p->batch_frames = (int32_t)mem_frames;
 
-    ts->tri_warps = tiled_warps(p, ts->tile_bins);
-    ts->tri_smem = tri_smem_bytes(ts->tile_bins, ts->tri_warps, n_r);
+    ts->tri_warps = tiled_warps(p, ts->slab_bins_max);
+    ts->tri_smem = tri_smem_bytes(ts->slab_bins_max, ts->tri_warps, n_r);
     ts->stage_cap = tiled_stage_cap(p);
     ts->nb_smem = nb_smem_bytes(ts->stage_cap, p->max_nb, n_r);
 
@@ -203,6 +257,12 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMalloc(&ts->d_nbv, sizeof(float4) * (per_frame_entries * B + 64)));   // +64: prefetch overrun
     G3T_CUDA(cudaMalloc(&ts->d_nbcount, sizeof(int32_t) * (size_t)p->n * B));
     G3T_CUDA(cudaMalloc(&ts->d_work, sizeof(unsigned int)));
+    if (ts->n_slabs > 1) {
+        G3T_CUDA(cudaMalloc(&ts->d_slab_shell, sizeof(int32_t) * (ts->n_slabs + 1)));
+        G3T_CUDA(cudaMemcpy(ts->d_slab_shell, ts->slab_shell.data(), sizeof(int32_t) * (ts->n_slabs + 1),
+                            cudaMemcpyHostToDevice));
+        G3T_CUDA(cudaMalloc(&ts->d_slabpos, sizeof(int32_t) * (size_t)p->n * B * (ts->n_slabs + 1)));
+    }
     {
         const int32_t nc = p->ncell;
         std::vector<int4> origin((size_t)nc * nc * nc);
@@ -258,6 +318,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     np.T_r = bs.T_r;
     np.cell_origin = ts->d_cell_origin;
     np.nbv = ts->d_nbv; np.nbcount = ts->d_nbcount; np.stats = p->d_stats;
+    np.n_slabs = ts->n_slabs; np.slab_shell = ts->d_slab_shell; np.slabpos = ts->d_slabpos;
     G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     if (p->timing) {
@@ -287,14 +348,24 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     tp.inv_hi = (float)((1.0 / wt) * (1.0 + eps));
     tp.T_t = bs.T_t; tp.nbv = ts->d_nbv; tp.nbcount = ts->d_nbcount;
     tp.addend = ts->d_addend; tp.jconst = ts->d_jconst;
-    tp.work = ts->d_work; tp.scratch = ts->d_scratch;
-    switch (ts->tri_warps) {
-        case 24: tiled_triplet_kernel<24><<<ts->grid, 24 * 32, ts->tri_smem, st>>>(tp); break;
-        case 16: tiled_triplet_kernel<16><<<ts->grid, 16 * 32, ts->tri_smem, st>>>(tp); break;
-        default: tiled_triplet_kernel<8><<<ts->grid, 8 * 32, ts->tri_smem, st>>>(tp); break;
+    tp.work = ts->d_work;
+    tp.scratch_stride = ts->tile_bins;
+    tp.n_slabs = ts->n_slabs; tp.slabpos = ts->d_slabpos;
+    for (int32_t s = 0; s < ts->n_slabs; ++s) {
+        const int32_t b0 = ts->slab_shell[s], b1 = ts->slab_shell[s + 1];
+        tp.slab = s;
+        tp.slot_base = ts->BASE[b0];
+        tp.tile_bins = ts->n_slabs > 1 ? ts->BASE[b1] - ts->BASE[b0] + 2 : (int32_t)ts->tile_bins;
+        tp.scratch = ts->d_scratch + tp.slot_base;
+        if (s > 0) G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
+        switch (ts->tri_warps) {
+            case 24: tiled_launch_triplet<24>(ts, tp, st); break;
+            case 16: tiled_launch_triplet<16>(ts, tp, st); break;
+            default: tiled_launch_triplet<8>(ts, tp, st); break;
+        }
     }
     if (p->timing) G3T_CUDA(cudaEventRecord(ev[2], st));
-    p->launches += 2;
+    p->launches += 1 + (uint64_t)ts->n_slabs;
     ts->dirty = true;
     G3T_CUDA(cudaGetLastError());
     return G3_OK;

@@ -40,7 +40,13 @@ struct TriParams {
     const float* addend;                  // [n_r]  kMagic + BASE(b) - g(b) + 1
     const int32_t* jconst;                // [n_r]  4 * (P(a) + h(a))
     unsigned int* work;
-    unsigned long long* scratch;          // [grid][tile_bins]
+    unsigned long long* scratch;          // [grid][scratch_stride], already offset by slot_base
+    // slab passes (kSlab kernels): this launch counts only pairs whose outer member k lies in
+    // the shell range of slab `slab`; its tile holds the slots slot_base+1 .. slot_base+tile_bins-2
+    long long scratch_stride;             // slots of the whole layout (= tile_bins without slabs)
+    int32_t slot_base;                    // BASE(first shell of the slab)
+    int32_t n_slabs, slab;
+    const int32_t* slabpos;               // [centres][n_slabs + 1] list position where each slab starts
 };
 
 __device__ __forceinline__ void red_shared_add(uint32_t addr, uint32_t v) {
@@ -181,7 +187,20 @@ __device__ __forceinline__ void triangle16(const TriParams& tp, const float4* __
                      kidx < kt, kidx + 4 < kt, k4 < kt, lane < 24 && kl < kt);
 }
 
-template <int kWarps>
+// Triangle of a 32-block whose k members are bounded below (slab passes): lane = j, the k
+// members klo <= k < kt are broadcast four at a time.  Runs at most once per centre and slab.
+__device__ __forceinline__ void triangle_from(const TriParams& tp, const float4* __restrict__ win,
+                                              uint32_t guard, int lane, int32_t klo, int32_t kt,
+                                              const JSide& own) {
+    for (int32_t k0 = klo; k0 < kt; k0 += 4) {
+        const float4 ka = win[k0], kb = win[min(k0 + 1, 31)], kc = win[min(k0 + 2, 31)], kd = win[min(k0 + 3, 31)];
+        four_pairs<true>(tp, guard, ka, kb, kc, kd, own, own, own, own,
+                         lane < k0, lane < k0 + 1 && k0 + 1 < kt, lane < k0 + 2 && k0 + 2 < kt,
+                         lane < k0 + 3 && k0 + 3 < kt);
+    }
+}
+
+template <int kWarps, bool kSlab>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 tiled_triplet_kernel(TriParams tp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -207,7 +226,7 @@ tiled_triplet_kernel(TriParams tp) {
     uint32_t* winJ = winJ_all + wid * 32;       // tile row offsets of winA's entries
     const uint32_t guard = (uint32_t)__cvta_generic_to_shared(tile);      // slot 0
     // shared-window byte address of slot 0 minus the magic bits (mod 2^32), see file header
-    const uint32_t cbase = guard - (kMagicBits << 2);
+    const uint32_t cbase = guard - (kMagicBits << 2) - (kSlab ? ((uint32_t)tp.slot_base << 2) : 0u);
     const long long n_items = (tp.total_centres + kItemCentres - 1) / kItemCentres;
 
     // work queue: a CTA first takes one of its own `cta_item_cap` tickets, then a global item
@@ -223,11 +242,15 @@ tiled_triplet_kernel(TriParams tp) {
         long long item_next = fetch_item();
         long long c = item * kItemCentres;
         long long c_end = min(c + (long long)kItemCentres, tp.total_centres);
-        int32_t Kn = tp.nbcount[c];
+        int32_t Kn = tp.nbcount[c], ksn = 0;
+        if (kSlab) {
+            const int32_t* sp = tp.slabpos + c * (tp.n_slabs + 1) + tp.slab;
+            ksn = sp[0]; Kn = sp[1];              // entries at or beyond the slab's end are not needed
+        }
         float4 v0n = tp.nbv[c * tp.max_nb + lane], v1n = tp.nbv[c * tp.max_nb + 32 + lane];
         bool more = true;
         while (more) {
-            const int32_t K = Kn;
+            const int32_t K = Kn, ks = ksn;
             const float4 v0 = v0n, v1 = v1n;
             const float4* __restrict__ lv = tp.nbv + c * tp.max_nb;
             // ---- advance and prefetch the next centre ------------------------------------------
@@ -240,11 +263,14 @@ tiled_triplet_kernel(TriParams tp) {
                 } else more = false;
             }
             if (more) {
-                Kn = tp.nbcount[c];
+                if (kSlab) {
+                    const int32_t* sp = tp.slabpos + c * (tp.n_slabs + 1) + tp.slab;
+                    ksn = sp[0]; Kn = sp[1];
+                } else Kn = tp.nbcount[c];
                 v0n = tp.nbv[c * tp.max_nb + lane];
                 v1n = tp.nbv[c * tp.max_nb + 32 + lane];
             }
-            if (K < 2) continue;
+            if (K < 2 || (kSlab && ks >= K)) continue;
 
             // ---- all unordered pairs of this centre's K neighbours ------------------------------
             const int32_t nchunks = (K + 31) >> 5;
@@ -258,8 +284,10 @@ tiled_triplet_kernel(TriParams tp) {
                 own.x = jvalid ? jraw.x : 0.f; own.y = jvalid ? jraw.y : 0.f; own.z = jvalid ? jraw.z : 0.f;
                 own.J = cbase + (uint32_t)tab_j[aj];
                 // prefetch the first rectangular window while the triangle runs
+                // (slab passes: the first k block is the one that holds list position ks)
+                const int32_t q_first = kSlab ? max(r + 1, ks >> 5) : r + 1;
                 float4 nextv = v1;
-                if (r + 1 >= 2 && r + 1 < nchunks && ((r + 1) << 5) + lane < K) nextv = lv[((r + 1) << 5) + lane];
+                if (q_first >= 2 && q_first < nchunks && (q_first << 5) + lane < K) nextv = lv[(q_first << 5) + lane];
 
                 // ---- triangle: both members in this 32-block -------------------------------------
                 __syncwarp();
@@ -267,7 +295,9 @@ tiled_triplet_kernel(TriParams tp) {
                 winJ[lane] = own.J;
                 __syncwarp();
                 const int32_t kt = min(32, K - (r << 5));
-                if (kt == 32) triangle32<true>(tp, winA, winJ, guard, lane, kt, own);
+                if (kSlab && ks > (r << 5)) {          // k members bounded below inside this block
+                    if (ks < (r << 5) + kt) triangle_from(tp, winA, guard, lane, ks - (r << 5), kt, own);
+                } else if (kt == 32) triangle32<true>(tp, winA, winJ, guard, lane, kt, own);
                 else if (kt > 16) triangle32<false>(tp, winA, winJ, guard, lane, kt, own);
                 else if (kt >= 2) triangle16(tp, winA, winJ, guard, lane, kt);
                 if (r + 1 == nchunks) break;
@@ -275,7 +305,7 @@ tiled_triplet_kernel(TriParams tp) {
                 // ---- rectangles: k in later 32-blocks; this block is full, 2 j x 2 k per lane ----
                 const int kg = lane >> 4;
                 const JSide ja = load_jside(winA, winJ, lane & 15), jb = load_jside(winA, winJ, (lane & 15) + 16);
-                for (int32_t q = r + 1; q < nchunks; ++q) {
+                for (int32_t q = q_first; q < nchunks; ++q) {
                     const bool kvalid = (q << 5) + lane < K;
                     const int32_t ak = kvalid ? __float_as_int(nextv.w) : 0;
                     __syncwarp();
@@ -284,21 +314,23 @@ tiled_triplet_kernel(TriParams tp) {
                     __syncwarp();
                     if (q + 1 < nchunks && ((q + 1) << 5) + lane < K) nextv = lv[((q + 1) << 5) + lane];
                     const int32_t kc = min(32, K - (q << 5));
-                    for (int32_t k0i = 0; k0i < kc; k0i += 4) {     // k = k0i + kg and k0i + kg + 2
+                    const int32_t klo = kSlab ? max(0, ks - (q << 5)) : 0;
+                    for (int32_t k0i = klo & ~3; k0i < kc; k0i += 4) {     // k = k0i + kg and k0i + kg + 2
                         const int32_t kidx = k0i + kg;
                         const float4 k0 = winB[kidx], k1 = winB[kidx + 2];
-                        if (k0i + 4 <= kc)
+                        if (k0i + 4 <= kc && (!kSlab || k0i >= klo))
                             four_pairs<false>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, true, true, true, true);
-                        else
-                            four_pairs<true>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb,
-                                             kidx < kc, kidx < kc, kidx + 2 < kc, kidx + 2 < kc);
+                        else {
+                            const bool pa = kidx < kc && kidx >= klo, pb = kidx + 2 < kc && kidx + 2 >= klo;
+                            four_pairs<true>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, pa, pa, pb, pb);
+                        }
                     }
                 }
             }
         }
     }
     __syncthreads();
-    unsigned long long* out = tp.scratch + (size_t)blockIdx.x * tp.tile_bins;
+    unsigned long long* out = tp.scratch + (size_t)blockIdx.x * (size_t)tp.scratch_stride;
     for (int32_t i = 1 + threadIdx.x; i < tp.tile_bins; i += blockDim.x) {
         const uint32_t v = tile[i];
         if (v) out[i] += v;

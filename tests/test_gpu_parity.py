@@ -70,6 +70,27 @@ def test_config5_one_frame(oracle_lib, g3, kernel):
     check(oracle_lib, g3, pos, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel)
 
 
+@pytest.mark.parametrize("n_r,n_t,max_nb", [(128, 128, None), (100, 200, None), (160, 96, 320)])
+def test_slab_passes(oracle_lib, g3, n_r, n_t, max_nb):
+    """bin counts whose reachable slots do not fit one shared-memory tile: the tiled kernel runs
+    one pass per slab of outer shells.  Water-like and clumped frames, so that
+    slab boundaries fall inside 32-blocks, on block edges and on empty shell ranges."""
+    import torch
+    w = WORKLOADS[2]
+    _, pos = frames(w, 3)
+    opts = {} if max_nb is None else {"max_neighbours": max_nb}
+    r_max = w.r_max if max_nb is None else 1.0
+    with g3.Plan(w.n, w.box, r_max, n_r, n_t, kernel=2, **opts) as plan:
+        assert plan.info(g3.G3_INFO_KERNEL) == 2 and plan.info(g3.G3_INFO_SLABS) > 1
+    check(oracle_lib, g3, pos, w.box, r_max, n_r, n_t, kernel=2, **opts)
+
+
+def test_config5_uses_slabs(g3):
+    w = WORKLOADS[5]
+    with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t) as plan:
+        assert plan.info(g3.G3_INFO_KERNEL) == 2 and plan.info(g3.G3_INFO_SLABS) > 1
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("n,box,r_max,n_r,n_t", [
     (3, 1.0, 0.4, 4, 4),            # smallest legal frame
