@@ -79,7 +79,7 @@ typedef enum {
     G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1)      */
     G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
     G3_OPT_MAX_NEIGHBOURS = 3, /* per-centre neighbour capacity (0 = derive from density)    */
-    G3_OPT_TRIPLET_WARPS = 5, /* warps per triplet-kernel CTA: 0 = auto, or 8 / 16 / 24        */
+    G3_OPT_TRIPLET_WARPS = 5, /* warps per triplet-kernel CTA: 0 = auto, or 8, 12, .. 24  */
     G3_OPT_TIMING = 4         /* 1 = bracket the neighbour and triplet kernels with CUDA events
                                  on the caller's stream (read back with g3_plan_get_info)     */
 } g3_option;

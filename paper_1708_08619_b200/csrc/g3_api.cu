@@ -272,7 +272,7 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
             if (value < 0 || value > (1 << 20)) return G3_EINVAL;
             p->max_nb_opt = (int32_t)value; break;
         case G3_OPT_TRIPLET_WARPS:
-            if (value != 0 && value != 8 && value != 16 && value != 24) return G3_EINVAL;
+            if (value != 0 && (value < 8 || value > 24 || value % 4 != 0)) return G3_EINVAL;
             p->tri_warps_opt = (int32_t)value; break;
         case G3_OPT_TIMING:
             if (value < 0 || value > 1) return G3_EINVAL;
@@ -345,30 +345,41 @@ int g3_accumulate_frames_host(g3_plan* p, const double* h_pos, int64_t n_frames,
     if (!p->d_h2d) {
         G3_CUDA(cudaMalloc(&p->d_h2d, 2 * chunk * frame_bytes));
         p->h2d_chunk_frames = chunk;
-        for (int i = 0; i < 2; ++i)
-            G3_CUDA(cudaEventCreateWithFlags(&p->h2d_done[i], cudaEventDisableTiming));
+        p->h2d_chunks = 0;
+        if (!p->copy_stream) {
+            G3_CUDA(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+            for (int i = 0; i < 2; ++i) {
+                G3_CUDA(cudaEventCreateWithFlags(&p->h2d_done[i], cudaEventDisableTiming));
+                G3_CUDA(cudaEventCreateWithFlags(&p->h2d_free[i], cudaEventDisableTiming));
+            }
+        }
     }
-    // Two device staging halves, all on the caller's stream: the copy of chunk c+1 is queued
-    // behind the quantise kernel of chunk c but ahead of its (much longer) triplet batch only
-    // when batches are flushed later; with pinned memory the copies run on the copy engine
-    // while earlier triplet kernels still occupy the SMs of other streams.  Kept simple and
-    // strictly ordered here: correctness does not depend on overlap.
-    int64_t done = 0, idx = 0;
+    // Two device staging halves.  The copies run on the plan's own copy stream (copy engine), the
+    // kernels on the caller's stream: the copy of chunk c+1 overlaps the neighbour/triplet
+    // kernels of chunk c.  h2d_done[h] orders copy -> quantise kernel, h2d_free[h] orders the
+    // kernels that read half h -> the next copy into it.  When the caller's stream has passed
+    // this call every copy has completed, so the include/g3.h lifetime rule for h_pos holds.
+    int64_t done = 0;
     while (done < n_frames) {
         const int64_t take = std::min(chunk, n_frames - done);
-        double* dst = p->d_h2d + (idx & 1) * chunk * 3 * p->n;
+        const int h = (int)(p->h2d_chunks & 1);
+        double* dst = p->d_h2d + (size_t)h * chunk * 3 * p->n;
+        if (p->h2d_chunks >= 2) G3_CUDA(cudaStreamWaitEvent(p->copy_stream, p->h2d_free[h], 0));
         if (frame_stride == 3 * p->n) {
             G3_CUDA(cudaMemcpyAsync(dst, h_pos + done * frame_stride, take * frame_bytes,
-                                    cudaMemcpyHostToDevice, st));
+                                    cudaMemcpyHostToDevice, p->copy_stream));
         } else {
             G3_CUDA(cudaMemcpy2DAsync(dst, frame_bytes, h_pos + done * frame_stride,
                                       sizeof(double) * frame_stride, frame_bytes, take,
-                                      cudaMemcpyHostToDevice, st));
+                                      cudaMemcpyHostToDevice, p->copy_stream));
         }
+        G3_CUDA(cudaEventRecord(p->h2d_done[h], p->copy_stream));
+        G3_CUDA(cudaStreamWaitEvent(st, p->h2d_done[h], 0));
         rc = accumulate_device(p, dst, take, 3 * p->n, st);
         if (rc != G3_OK) return rc;
+        G3_CUDA(cudaEventRecord(p->h2d_free[h], st));
+        p->h2d_chunks += 1;
         done += take;
-        ++idx;
     }
     return G3_OK;
 }
@@ -454,8 +465,11 @@ void g3_plan_destroy(g3_plan* p) {
     if (!p) return;
     cudaDeviceSynchronize();
     free_buffers(p);
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < 2; ++i) {
         if (p->h2d_done[i]) cudaEventDestroy(p->h2d_done[i]);
+        if (p->h2d_free[i]) cudaEventDestroy(p->h2d_free[i]);
+    }
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
     cudaFree(p->d_T_r); cudaFree(p->d_T_t); cudaFree(p->d_counts); cudaFree(p->d_stats);
     cudaFree(p->d_volumes);

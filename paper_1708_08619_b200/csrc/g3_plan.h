@@ -73,8 +73,11 @@ struct g3_plan {
     int32_t* d_cell_start = nullptr;         // [batch][ncell3 + 1]
     int4* d_sorted = nullptr;                // [batch][n]
     double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
-    cudaEvent_t h2d_done[2] = {nullptr, nullptr};
+    cudaEvent_t h2d_done[2] = {nullptr, nullptr};   // copy of a staging half finished (copy stream)
+    cudaEvent_t h2d_free[2] = {nullptr, nullptr};   // staging half consumed (caller's stream)
+    cudaStream_t copy_stream = nullptr;             // host->device copies overlap the kernels
     int64_t h2d_chunk_frames = 0;
+    uint64_t h2d_chunks = 0;                        // chunks copied so far (selects the half)
     // G3_OPT_TIMING: event triples (before neighbour, between, after triplet) per launch pair
     std::vector<cudaEvent_t> ev_pool;        // all events ever created (reused after a clear)
     size_t ev_used = 0;                      // events of ev_pool recorded since the last clear

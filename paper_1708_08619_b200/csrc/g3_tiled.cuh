@@ -129,8 +129,8 @@ inline int32_t tiled_stage_cap(const g3_plan* p) {
 }
 
 inline int tiled_warps(const g3_plan* p, int64_t tile_bins) {
-    int w = p->tri_warps_opt ? p->tri_warps_opt : 24;
-    while (w > 8 && tri_smem_bytes(tile_bins, w, p->bins.n_r) > (size_t)p->smem_optin) w -= 8;
+    int w = p->tri_warps_opt ? p->tri_warps_opt : 20;   // 20 warps x 96 registers: no spills (measured best)
+    while (w > 8 && tri_smem_bytes(tile_bins, w, p->bins.n_r) > (size_t)p->smem_optin) w -= 4;
     return w;
 }
 
@@ -150,7 +150,7 @@ inline bool tiled_plan_slabs(const g3_plan* p, TiledState& ts) {
         ts.slab_bins_max = ts.tile_bins;
         return true;
     }
-    const int warps = p->tri_warps_opt ? p->tri_warps_opt : 24;
+    const int warps = p->tri_warps_opt ? p->tri_warps_opt : 20;
     return build_slabs(ts, p->bins.n_r, tiled_cap_slots(p, warps)) && ts.n_slabs <= 64;
 }
 
@@ -285,6 +285,8 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
     switch (ts->tri_warps) {
         case 24: return tiled_set_attr<24>(ts->tri_smem);
+        case 20: return tiled_set_attr<20>(ts->tri_smem);
+        case 12: return tiled_set_attr<12>(ts->tri_smem);
         case 16: return tiled_set_attr<16>(ts->tri_smem);
         default: return tiled_set_attr<8>(ts->tri_smem);
     }
@@ -360,6 +362,8 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         if (s > 0) G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
         switch (ts->tri_warps) {
             case 24: tiled_launch_triplet<24>(ts, tp, st); break;
+            case 20: tiled_launch_triplet<20>(ts, tp, st); break;
+            case 12: tiled_launch_triplet<12>(ts, tp, st); break;
             case 16: tiled_launch_triplet<16>(ts, tp, st); break;
             default: tiled_launch_triplet<8>(ts, tp, st); break;
         }
