@@ -362,6 +362,42 @@ void g3o_normalise(const uint64_t *H, const double *V, int64_t nbins,
         g3[b] = V[b] > 0.0 ? (double)H[b] / (ideal * V[b]) : 0.0;
 }
 
+/* ------------------------------------------------------------------------- */
+/* g2: the pair distribution function from the same pair loop.
+ * Algorithm 6 computes it beside the neighbour vectors ("Calculate the minimum image
+ * distance ... Update the g2 histogram") and Algorithm 7's CUDA_g2 kernel
+ * does the same per thread i.  Reading G1: the paper's g2
+ * cut-off is L/2; here the pair histogram covers the neighbour range [0, r_max) with the n_r
+ * shells of r_ij, i.e. H2[a] = number of ORDERED pairs (i, j), j != i, whose minimum-image
+ * squared distance falls in [T_r[a], T_r[a+1]).  Plain all-pairs double loop, no cell list.
+ * H2 [n_r] is ADDED to.  Pins: tests/test_oracle_g2.py.                                    */
+void g3o_g2_frame(const int32_t *m, int64_t n, const uint64_t *T_r, int32_t n_r, uint64_t *H2)
+{
+    for (int64_t i = 0; i < n; ++i)
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            int64_t dx = wrap((int64_t)m[3 * j + 0] - m[3 * i + 0]);
+            int64_t dy = wrap((int64_t)m[3 * j + 1] - m[3 * i + 1]);
+            int64_t dz = wrap((int64_t)m[3 * j + 2] - m[3 * i + 2]);
+            uint64_t d2 = (uint64_t)(dx * dx + dy * dy + dz * dz);
+            if (d2 < T_r[n_r]) H2[bin_of(T_r, n_r, d2)] += 1;
+        }
+}
+
+/* g2[a] = H2[a] / (F N rho V_a), V_a = (4 pi / 3)(r_{a+1}^3 - r_a^3), rho = N / L^3: the
+ * ideal-gas value is (N-1)/N (same rho convention as Eq. 3, reading Q9).                   */
+void g3o_g2_normalise(const uint64_t *H2, int32_t n_r, double r_max, int64_t n_frames, int64_t n,
+                      double box, double *g2)
+{
+    double rho = (double)n / (box * box * box);
+    double w = r_max / (double)n_r;
+    for (int32_t a = 0; a < n_r; ++a) {
+        double r0 = a * w, r1 = (a + 1) * w;
+        double V = (4.0 * 3.14159265358979323846 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0);
+        g2[a] = n_frames > 0 ? (double)H2[a] / ((double)n_frames * (double)n * rho * V) : 0.0;
+    }
+}
+
 int32_t g3o_num_threads(void)
 {
 #ifdef _OPENMP

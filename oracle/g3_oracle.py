@@ -41,6 +41,10 @@ def _load() -> C.CDLL:
                                         C.c_int32, C.c_int32, C.c_int32, u64p, u64p]
         _lib.g3o_volumes.argtypes = [C.c_double, C.c_int32, C.c_int32, f64p]
         _lib.g3o_normalise.argtypes = [u64p, f64p, C.c_int64, C.c_int64, C.c_int64, C.c_double, f64p]
+        _lib.g3o_g2_frame.argtypes = [i32p, C.c_int64, u64p, C.c_int32, u64p]
+        _lib.g3o_g2_frame.restype = None
+        _lib.g3o_g2_normalise.argtypes = [u64p, C.c_int32, C.c_double, C.c_int64, C.c_int64, C.c_double, f64p]
+        _lib.g3o_g2_normalise.restype = None
         _lib.g3o_num_threads.restype = C.c_int32
         for fn in (_lib.g3o_thresholds, _lib.g3o_quantise, _lib.g3o_accumulate, _lib.g3o_volumes,
                    _lib.g3o_normalise):
@@ -124,6 +128,24 @@ def normalise(H: np.ndarray, V: np.ndarray, n_frames: int, n: int, box: float) -
     _load().g3o_normalise(_p(H, C.c_uint64), _p(V, C.c_double), H.size, n_frames, n, box,
                           _p(g3, C.c_double))
     return g3
+
+
+def g2_frame(m: np.ndarray, T_r: np.ndarray, H2: Optional[np.ndarray] = None) -> np.ndarray:
+    """Add one frame's ordered-pair counts per r_ij shell to H2 [n_r] (g3o_g2_frame)."""
+    m = np.ascontiguousarray(m, dtype=np.int32)
+    T_r = np.ascontiguousarray(T_r, dtype=np.uint64)
+    n_r = T_r.size - 1
+    if H2 is None:
+        H2 = np.zeros(n_r, dtype=np.uint64)
+    _load().g3o_g2_frame(_p(m, C.c_int32), m.shape[0], _p(T_r, C.c_uint64), n_r, _p(H2, C.c_uint64))
+    return H2
+
+
+def g2_normalise(H2: np.ndarray, r_max: float, n_frames: int, n: int, box: float) -> np.ndarray:
+    H2 = np.ascontiguousarray(H2, dtype=np.uint64)
+    g2 = np.zeros(H2.size, dtype=np.float64)
+    _load().g3o_g2_normalise(_p(H2, C.c_uint64), H2.size, r_max, n_frames, n, box, _p(g2, C.c_double))
+    return g2
 
 
 class Oracle:
