@@ -161,6 +161,16 @@ G3_API int g3_finalize(g3_plan *p, uint64_t *d_counts, double *d_g3, uint64_t *h
 /* Same with HOST output buffers (device-to-host copies included).                   */
 G3_API int g3_finalize_host(g3_plan *p, uint64_t *h_counts, double *h_g3, uint64_t *h_stats, void *stream);
 
+/* g2, the pair distribution function, from the same neighbour pass (Algorithm 6 "g2
+ * histogram"; Algorithm 7 CUDA_g2; reading G1:
+ * the range is the neighbour range [0, r_max) with the n_r shells of r_ij, not the paper's
+ * L/2).  Reduces all staged frames like g3_finalize, then, asynchronously on `stream`:
+ *   d_counts2  device, uint64 [n_r]: ordered pairs (i, j), j != i, per shell; may be NULL
+ *   d_g2       device, fp64 [n_r]: counts2 / (frames n rho V_a), V_a = 4 pi/3 (r_{a+1}^3 - r_a^3),
+ *              rho = n / box^3 (ideal gas -> (n-1)/n); may be NULL
+ * Does not synchronise and does not reset.  sum(counts2) = sum_i k_i.                */
+G3_API int g3_finalize_g2(g3_plan *p, uint64_t *d_counts2, double *d_g2, void *stream);
+
 /* Normalise externally merged counts (e.g. the sum over ranks of a frame-sharded
  * run; the paper's "split the trajectory, merge the results"):
  * d_g3 = d_counts / (frames n rho^2 V_abc).  Asynchronous on `stream`.              */

@@ -373,15 +373,25 @@ void g3o_normalise(const uint64_t *H, const double *V, int64_t nbins,
  * H2 [n_r] is ADDED to.  Pins: tests/test_oracle_g2.py.                                    */
 void g3o_g2_frame(const int32_t *m, int64_t n, const uint64_t *T_r, int32_t n_r, uint64_t *H2)
 {
-    for (int64_t i = 0; i < n; ++i)
-        for (int64_t j = 0; j < n; ++j) {
-            if (j == i) continue;
-            int64_t dx = wrap((int64_t)m[3 * j + 0] - m[3 * i + 0]);
-            int64_t dy = wrap((int64_t)m[3 * j + 1] - m[3 * i + 1]);
-            int64_t dz = wrap((int64_t)m[3 * j + 2] - m[3 * i + 2]);
-            uint64_t d2 = (uint64_t)(dx * dx + dy * dy + dz * dz);
-            if (d2 < T_r[n_r]) H2[bin_of(T_r, n_r, d2)] += 1;
-        }
+    /* OpenMP splits the centres i over threads, one private histogram each, summed at the end
+     * (integer sums: the result does not depend on the split).                              */
+#pragma omp parallel
+    {
+        uint64_t *h = (uint64_t *)calloc((size_t)n_r, sizeof(uint64_t));
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t j = 0; j < n; ++j) {
+                if (j == i) continue;
+                int64_t dx = wrap((int64_t)m[3 * j + 0] - m[3 * i + 0]);
+                int64_t dy = wrap((int64_t)m[3 * j + 1] - m[3 * i + 1]);
+                int64_t dz = wrap((int64_t)m[3 * j + 2] - m[3 * i + 2]);
+                uint64_t d2 = (uint64_t)(dx * dx + dy * dy + dz * dz);
+                if (d2 < T_r[n_r]) h[bin_of(T_r, n_r, d2)] += 1;
+            }
+#pragma omp critical
+        for (int32_t a = 0; a < n_r; ++a) H2[a] += h[a];
+        free(h);
+    }
 }
 
 /* g2[a] = H2[a] / (F N rho V_a), V_a = (4 pi / 3)(r_{a+1}^3 - r_a^3), rho = N / L^3: the

@@ -23,7 +23,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_normalize", "g3_bin_volumes", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_normalize", "g3_bin_volumes", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -59,6 +59,7 @@ def load() -> C.CDLL:
     lib.g3_accumulate_frames_host.argtypes = [vp, vp, i64, i64, vp]
     lib.g3_finalize.argtypes = [vp, vp, vp, vp, vp]
     lib.g3_finalize_host.argtypes = [vp, vp, vp, vp, vp]
+    lib.g3_finalize_g2.argtypes = [vp, vp, vp, vp]
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
     lib.g3_plan_reset.argtypes = [vp, vp]
@@ -174,6 +175,15 @@ class Plan:
         _check(self._lib.g3_finalize_host(self._h, counts.data_ptr(), g3.data_ptr() if want_g3 else None,
                                           stats, _stream_ptr(stream)), "g3_finalize_host")
         return counts, g3, [int(v) for v in stats]
+
+    def finalize_g2(self, stream=None):
+        """(counts2 int64-viewed-as-uint64 [n_r], g2 fp64 [n_r]) device tensors; stream-ordered."""
+        import torch
+        counts2 = torch.empty(self.n_r, dtype=torch.int64, device="cuda")
+        g2 = torch.empty(self.n_r, dtype=torch.float64, device="cuda")
+        _check(self._lib.g3_finalize_g2(self._h, counts2.data_ptr(), g2.data_ptr(), _stream_ptr(stream)),
+               "g3_finalize_g2")
+        return counts2, g2
 
     def normalize(self, d_counts, frames: int, stream=None):
         import torch

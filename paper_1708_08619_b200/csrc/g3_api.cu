@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "g3_cells.cuh"
 #include "g3_generic.cuh"
@@ -46,6 +47,15 @@ normalise_kernel(const unsigned long long* __restrict__ counts, const double* __
     double v = volumes[b];
     // g3 = H / (F N rho^2 V_abc); 0 where V_abc = 0.  inv_ideal = 1 / (F N rho^2).
     g3out[b] = v > 0.0 ? __ddiv_rn(__dmul_rn((double)counts[b], inv_ideal), v) : 0.0;
+}
+
+__global__ void __launch_bounds__(256)
+normalise_g2_kernel(const unsigned long long* __restrict__ counts2, const double* __restrict__ shell_volumes,
+                    int32_t n_r, double inv_ideal, double* __restrict__ g2out) {
+    int32_t a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n_r) return;
+    // g2 = H2 / (F N rho V_a); inv_ideal = 1 / (F N rho)
+    g2out[a] = __ddiv_rn(__dmul_rn((double)counts2[a], inv_ideal), shell_volumes[a]);
 }
 
 void free_buffers(g3_plan* p) {
@@ -134,7 +144,7 @@ int flush(g3_plan* p, cudaStream_t st) {
         long long blocks = std::min<long long>((total + kGenericWarps - 1) / kGenericWarps,
                                                (long long)p->sm_count * 32);
         generic_triplet_kernel<kGenericWarps><<<(unsigned)blocks, kGenericWarps * 32, smem, st>>>(
-            fb, bs, p->max_nb, p->d_counts, p->d_stats);
+            fb, bs, p->max_nb, p->d_counts, p->d_counts2, p->d_stats);
         p->launches += 1;
     } else {
         int rc = tiled_launch(p, fb, bs, st);
@@ -247,6 +257,18 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
     G3_TRY(cudaMalloc(&p->d_T_t, sizeof(unsigned long long) * p->T_t.size()));
     G3_TRY(cudaMalloc(&p->d_counts, sizeof(unsigned long long) * p->nbins));
     G3_TRY(cudaMalloc(&p->d_stats, sizeof(unsigned long long) * 4));
+    G3_TRY(cudaMalloc(&p->d_counts2, sizeof(unsigned long long) * bins.n_r));
+    G3_TRY(cudaMemset(p->d_counts2, 0, sizeof(unsigned long long) * bins.n_r));
+    {   // shell volumes V_a = (4 pi / 3)(r_{a+1}^3 - r_a^3) for g2
+        std::vector<double> v2(bins.n_r);
+        const double w = r_max / (double)bins.n_r;
+        for (int32_t a = 0; a < bins.n_r; ++a) {
+            const double r0 = a * w, r1 = (a + 1) * w;
+            v2[a] = (4.0 * 3.14159265358979323846 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0);
+        }
+        G3_TRY(cudaMalloc(&p->d_volumes2, sizeof(double) * bins.n_r));
+        G3_TRY(cudaMemcpy(p->d_volumes2, v2.data(), sizeof(double) * bins.n_r, cudaMemcpyHostToDevice));
+    }
     G3_TRY(cudaMalloc(&p->d_volumes, sizeof(double) * p->nbins));
     G3_TRY(cudaMemcpy(p->d_T_r, p->T_r.data(), sizeof(unsigned long long) * p->T_r.size(), cudaMemcpyHostToDevice));
     G3_TRY(cudaMemcpy(p->d_T_t, p->T_t.data(), sizeof(unsigned long long) * p->T_t.size(), cudaMemcpyHostToDevice));
@@ -419,6 +441,29 @@ int g3_finalize(g3_plan* p, uint64_t* d_counts, double* d_g3, uint64_t* h_stats,
     return stats[2] ? G3_ECAPACITY : G3_OK;
 }
 
+int g3_finalize_g2(g3_plan* p, uint64_t* d_counts2, double* d_g2, void* stream) {
+    if (!p) return G3_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = configure(p);
+    if (rc != G3_OK) return rc;
+    rc = flush(p, st);
+    if (rc != G3_OK) return rc;
+    rc = tiled_merge(p, st);
+    if (rc != G3_OK) return rc;
+    const int32_t n_r = p->bins.n_r;
+    if (d_counts2)
+        G3_CUDA(cudaMemcpyAsync(d_counts2, p->d_counts2, sizeof(uint64_t) * n_r, cudaMemcpyDeviceToDevice, st));
+    if (d_g2) {
+        const double rho = (double)p->n / (p->box * p->box * p->box);
+        const double ideal = (double)p->frames * (double)p->n * rho;
+        normalise_g2_kernel<<<(unsigned)((n_r + 255) / 256), 256, 0, st>>>(
+            p->d_counts2, p->d_volumes2, n_r, p->frames ? 1.0 / ideal : 0.0, d_g2);
+        p->launches += 1;
+        G3_CUDA(cudaGetLastError());
+    }
+    return G3_OK;
+}
+
 int g3_finalize_host(g3_plan* p, uint64_t* h_counts, double* h_g3, uint64_t* h_stats, void* stream) {
     if (!p) return G3_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -447,13 +492,14 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     G3_CUDA(cudaMemsetAsync(p->d_counts, 0, sizeof(unsigned long long) * p->nbins, st));
     G3_CUDA(cudaMemsetAsync(p->d_stats, 0, sizeof(unsigned long long) * 4, st));
+    G3_CUDA(cudaMemsetAsync(p->d_counts2, 0, sizeof(unsigned long long) * p->bins.n_r, st));
     if (p->configured && p->pending) {
         const size_t nc3 = (size_t)p->ncell * p->ncell * p->ncell;
         G3_CUDA(cudaMemsetAsync(p->d_cell_count, 0, sizeof(int32_t) * p->batch_frames * nc3, st));
     }
     if (p->tiled) {
         G3_CUDA(cudaMemsetAsync(p->tiled->d_scratch, 0,
-                                sizeof(unsigned long long) * p->tiled->tile_bins * p->tiled->grid, st));
+                                sizeof(unsigned long long) * (p->tiled->tile_bins + p->bins.n_r) * p->tiled->grid, st));
         p->tiled->dirty = false;
     }
     p->pending = 0;
@@ -472,7 +518,7 @@ void g3_plan_destroy(g3_plan* p) {
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
     cudaFree(p->d_T_r); cudaFree(p->d_T_t); cudaFree(p->d_counts); cudaFree(p->d_stats);
-    cudaFree(p->d_volumes);
+    cudaFree(p->d_volumes); cudaFree(p->d_counts2); cudaFree(p->d_volumes2);
     cudaGetLastError();
     delete p;
 }

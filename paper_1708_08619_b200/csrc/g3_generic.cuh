@@ -67,6 +67,7 @@ template <int kWarps>
 __global__ void __launch_bounds__(kWarps * 32)
 generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb,
                        unsigned long long* __restrict__ counts,
+                       unsigned long long* __restrict__ counts2,
                        unsigned long long* __restrict__ stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned long long* sT_r = reinterpret_cast<unsigned long long*>(smem_raw);
@@ -120,9 +121,10 @@ generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb,
         __syncwarp();
         if (lane == 0) my_pairs += (unsigned long long)count * (unsigned long long)(count - 1);
 
-        // a4: ordered pairs (j, k), j != k
+        // a4: ordered pairs (j, k), j != k; g2: one count per neighbour in its shell
         for (int32_t j = lane; j < count; j += 32) {
             const int4 vj = nb[j];
+            atomicAdd(counts2 + vj.w, 1ull);
             unsigned long long* row = counts + (size_t)vj.w * bs.n_r * bs.n_t;
             for (int32_t k = 0; k < count; ++k) {
                 if (k == j) continue;

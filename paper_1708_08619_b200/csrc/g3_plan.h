@@ -65,8 +65,10 @@ struct g3_plan {
     unsigned long long* d_T_r = nullptr;
     unsigned long long* d_T_t = nullptr;
     unsigned long long* d_counts = nullptr;  // [nbins] running histogram (ordered pairs)
+    unsigned long long* d_counts2 = nullptr; // [n_r] g2: ordered pairs (i, j) per shell of r_ij
     unsigned long long* d_stats = nullptr;   // [4]: pairs, overflow, capacity error, spare
     double* d_volumes = nullptr;             // [nbins]
+    double* d_volumes2 = nullptr;            // [n_r] shell volumes for g2
     int4* d_staged = nullptr;                // [batch][n] quantised (x,y,z,cell) in input order
     int32_t* d_slot = nullptr;               // [batch][n] rank of the particle inside its cell
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]

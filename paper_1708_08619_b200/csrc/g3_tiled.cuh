@@ -253,7 +253,7 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMalloc(&ts->d_addend, sizeof(float) * n_r));
     G3T_CUDA(cudaMalloc(&ts->d_jconst, sizeof(int32_t) * n_r));
     G3T_CUDA(cudaMalloc(&ts->d_slot_map, sizeof(uint32_t) * ts->tile_bins));
-    G3T_CUDA(cudaMalloc(&ts->d_scratch, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
+    G3T_CUDA(cudaMalloc(&ts->d_scratch, sizeof(unsigned long long) * (ts->tile_bins + n_r) * ts->grid));
     G3T_CUDA(cudaMalloc(&ts->d_nbv, sizeof(float4) * (per_frame_entries * B + 64)));   // +64: prefetch overrun
     G3T_CUDA(cudaMalloc(&ts->d_nbcount, sizeof(int32_t) * (size_t)p->n * B));
     G3T_CUDA(cudaMalloc(&ts->d_work, sizeof(unsigned int)));
@@ -279,7 +279,7 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMemcpy(ts->d_addend, addend.data(), sizeof(float) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_jconst, jconst.data(), sizeof(int32_t) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_slot_map, slot_map.data(), sizeof(uint32_t) * ts->tile_bins, cudaMemcpyHostToDevice));
-    G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
+    G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * (ts->tile_bins + n_r) * ts->grid));
     G3T_CUDA(cudaMemset(ts->d_nbv, 0, sizeof(float4) * (per_frame_entries * B + 64)));
     G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
     G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
@@ -295,9 +295,9 @@ inline int tiled_configure(g3_plan* p) {
 inline int tiled_merge(g3_plan* p, cudaStream_t st) {
     TiledState* ts = p->tiled;
     if (!ts || !ts->dirty) return G3_OK;
-    merge_kernel<<<(unsigned)((ts->tile_bins + 255) / 256), 256, 0, st>>>(
+    merge_kernel<<<(unsigned)((ts->tile_bins + p->bins.n_r + 255) / 256), 256, 0, st>>>(
         ts->d_scratch, ts->d_slot_map, (int32_t)ts->tile_bins, ts->grid, p->bins.n_r, p->bins.n_t,
-        p->d_counts, p->d_stats);
+        p->d_counts, p->d_counts2, p->d_stats);
     p->launches += 1;
     ts->dirty = false;
     G3T_CUDA(cudaGetLastError());
@@ -351,7 +351,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     tp.T_t = bs.T_t; tp.nbv = ts->d_nbv; tp.nbcount = ts->d_nbcount;
     tp.addend = ts->d_addend; tp.jconst = ts->d_jconst;
     tp.work = ts->d_work;
-    tp.scratch_stride = ts->tile_bins;
+    tp.scratch_stride = ts->tile_bins + bs.n_r;
     tp.n_slabs = ts->n_slabs; tp.slabpos = ts->d_slabpos;
     for (int32_t s = 0; s < ts->n_slabs; ++s) {
         const int32_t b0 = ts->slab_shell[s], b1 = ts->slab_shell[s + 1];
@@ -359,6 +359,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         tp.slot_base = ts->BASE[b0];
         tp.tile_bins = ts->n_slabs > 1 ? ts->BASE[b1] - ts->BASE[b0] + 2 : (int32_t)ts->tile_bins;
         tp.scratch = ts->d_scratch + tp.slot_base;
+        tp.g2_out = ts->tile_bins - tp.slot_base;
         if (s > 0) G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
         switch (ts->tri_warps) {
             case 24: tiled_launch_triplet<24>(ts, tp, st); break;

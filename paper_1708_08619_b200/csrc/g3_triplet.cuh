@@ -43,7 +43,8 @@ struct TriParams {
     unsigned long long* scratch;          // [grid][scratch_stride], already offset by slot_base
     // slab passes (kSlab kernels): this launch counts only pairs whose outer member k lies in
     // the shell range of slab `slab`; its tile holds the slots slot_base+1 .. slot_base+tile_bins-2
-    long long scratch_stride;             // slots of the whole layout (= tile_bins without slabs)
+    long long scratch_stride;             // slots of one CTA's partial tile: whole layout + n_r (g2)
+    long long g2_out;                     // offset of the g2 slots from `scratch` (pre-offset pointer)
     int32_t slot_base;                    // BASE(first shell of the slab)
     int32_t n_slabs, slab;
     const int32_t* slabpos;               // [centres][n_slabs + 1] list position where each slab starts
@@ -205,14 +206,15 @@ __global__ void __launch_bounds__(kWarps * 32, 1)
 tiled_triplet_kernel(TriParams tp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t* tile = reinterpret_cast<uint32_t*>(smem_raw);
-    const size_t tile_bytes = ((size_t)tp.tile_bins * 4 + 15) & ~size_t(15);
+    const size_t tile_bytes = ((size_t)(tp.tile_bins + tp.n_r) * 4 + 15) & ~size_t(15);
     float4* win_all = reinterpret_cast<float4*>(smem_raw + tile_bytes);       // [warp][2][32]
     uint32_t* winJ_all = reinterpret_cast<uint32_t*>(win_all + kWarps * 64);  // [warp][32]
     float* tab_addend = reinterpret_cast<float*>(winJ_all + kWarps * 32);
     int32_t* tab_j = reinterpret_cast<int32_t*>(tab_addend + tp.n_r);
     __shared__ unsigned int cta_items;
 
-    for (int32_t i = threadIdx.x; i < tp.tile_bins; i += blockDim.x) tile[i] = 0;
+    // the n_r slots after the tile count this CTA's neighbours per shell (g2)
+    for (int32_t i = threadIdx.x; i < tp.tile_bins + tp.n_r; i += blockDim.x) tile[i] = 0;
     for (int32_t i = threadIdx.x; i < tp.n_r; i += blockDim.x) {
         tab_addend[i] = tp.addend[i];
         tab_j[i] = tp.jconst[i];
@@ -227,6 +229,7 @@ tiled_triplet_kernel(TriParams tp) {
     const uint32_t guard = (uint32_t)__cvta_generic_to_shared(tile);      // slot 0
     // shared-window byte address of slot 0 minus the magic bits (mod 2^32), see file header
     const uint32_t cbase = guard - (kMagicBits << 2) - (kSlab ? ((uint32_t)tp.slot_base << 2) : 0u);
+    const uint32_t g2base = guard + ((uint32_t)tp.tile_bins << 2);
     const long long n_items = (tp.total_centres + kItemCentres - 1) / kItemCentres;
 
     // work queue: a CTA first takes one of its own `cta_item_cap` tickets, then a global item
@@ -270,7 +273,11 @@ tiled_triplet_kernel(TriParams tp) {
                 v0n = tp.nbv[c * tp.max_nb + lane];
                 v1n = tp.nbv[c * tp.max_nb + 32 + lane];
             }
-            if (K < 2 || (kSlab && ks >= K)) continue;
+            if (K < 2 || (kSlab && ks >= K)) {
+                if (K == 1 && ks == 0)           // a single neighbour: no pair, but one g2 count
+                    red_shared_add(lane == 0 ? g2base + ((uint32_t)__float_as_int(v0.w) << 2) : guard, 1u);
+                continue;
+            }
 
             // ---- all unordered pairs of this centre's K neighbours ------------------------------
             const int32_t nchunks = (K + 31) >> 5;
@@ -283,6 +290,7 @@ tiled_triplet_kernel(TriParams tp) {
                 JSide own;
                 own.x = jvalid ? jraw.x : 0.f; own.y = jvalid ? jraw.y : 0.f; own.z = jvalid ? jraw.z : 0.f;
                 own.J = cbase + (uint32_t)tab_j[aj];
+                red_shared_add(jvalid && (!kSlab || jidx >= ks) ? g2base + ((uint32_t)aj << 2) : guard, 1u);
                 // prefetch the first rectangular window while the triangle runs
                 // (slab passes: the first k block is the one that holds list position ks)
                 const int32_t q_first = kSlab ? max(r + 1, ks >> 5) : r + 1;
@@ -335,6 +343,10 @@ tiled_triplet_kernel(TriParams tp) {
         const uint32_t v = tile[i];
         if (v) out[i] += v;
     }
+    for (int32_t a = threadIdx.x; a < tp.n_r; a += blockDim.x) {
+        const uint32_t v = tile[tp.tile_bins + a];
+        if (v) out[tp.g2_out + a] += v;
+    }
 }
 
 // Mirror the per-CTA partial tiles into the uint64 histogram (step a5) and clear them.
@@ -342,16 +354,18 @@ tiled_triplet_kernel(TriParams tp) {
 __global__ void __launch_bounds__(256)
 merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restrict__ slot_map,
              int32_t tile_bins, int32_t grid, int32_t n_r, int32_t n_t,
-             unsigned long long* __restrict__ counts, unsigned long long* __restrict__ stats) {
+             unsigned long long* __restrict__ counts, unsigned long long* __restrict__ counts2,
+             unsigned long long* __restrict__ stats) {
     const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= tile_bins) return;
+    if (i >= tile_bins + n_r) return;
     unsigned long long v = 0;
     for (int32_t gidx = 0; gidx < grid; ++gidx) {
-        unsigned long long* p = scratch + (size_t)gidx * tile_bins + i;
+        unsigned long long* p = scratch + (size_t)gidx * (tile_bins + n_r) + i;
         const unsigned long long x = *p;
         if (x) { v += x; *p = 0; }
     }
     if (v == 0) return;
+    if (i >= tile_bins) { counts2[i - tile_bins] += v; return; }      // g2 slots
     const uint32_t m = slot_map[i];
     if (m == 0xFFFFFFFFu) { atomicAdd(stats + 3, v); return; }      // must never happen
     const int32_t a = (int32_t)(m >> 21), b = (int32_t)((m >> 11) & 1023), c = (int32_t)(m & 2047);
@@ -364,7 +378,7 @@ merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restric
 }
 
 inline size_t tri_smem_bytes(int64_t tile_bins, int warps, int32_t n_r) {
-    return (((size_t)tile_bins * 4 + 15) & ~size_t(15)) + (size_t)warps * (64 * 16 + 32 * 4) + (size_t)n_r * 8;
+    return (((size_t)(tile_bins + n_r) * 4 + 15) & ~size_t(15)) + (size_t)warps * (64 * 16 + 32 * 4) + (size_t)n_r * 8;
 }
 
 }  // namespace g3

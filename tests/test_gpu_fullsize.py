@@ -66,6 +66,28 @@ def test_full_trajectory_bit_exact(oracle_lib, g3, widx):
         assert np.array_equal(H, Ho)
         assert int(H.sum()) == stats[1]
         check_g3(oracle_lib, w, H, G.cpu().numpy(), w.n_frames)
+        # g2 of the whole trajectory; the O(N^2) oracle runs every frame (every 25th for config 4)
+        c2, g2 = plan.finalize_g2()
+        c2 = c2.cpu().numpy().view(np.uint64)
+        T_r, _ = oracle_lib.thresholds(w.box, w.r_max, w.n_r, w.n_t)
+        if widx != 4:
+            H2 = np.zeros(w.n_r, dtype=np.uint64)
+            for m in ms:
+                oracle_lib.g2_frame(m, T_r, H2)
+            assert np.array_equal(c2, H2)
+            assert np.allclose(g2.cpu().numpy(), oracle_lib.g2_normalise(H2, w.r_max, w.n_frames, w.n, w.box),
+                               rtol=G3_RTOL, atol=0)
+        else:
+            with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t) as p2:
+                H2 = np.zeros(w.n_r, dtype=np.uint64)
+                for f in range(0, w.n_frames, 25):
+                    p2.accumulate_frame(d_pos[f])
+                    oracle_lib.g2_frame(ms[f], T_r, H2)
+                s2, _ = p2.finalize_g2()
+                assert np.array_equal(s2.cpu().numpy().view(np.uint64), H2)
+        # sum_a counts2[a] = sum_i k_i; Cauchy-Schwarz ties it to the triplet statistic
+        k_sum = int(c2.sum())
+        assert stats[1] + k_sum >= k_sum * k_sum // (w.n * w.n_frames)
         plan.reset()                                                         # the e2e leg
         plan.accumulate_frames_host(h_pos)
         hc, hg, hs = plan.finalize_host()
@@ -86,20 +108,35 @@ def test_full_trajectory_sampled(oracle_lib, g3, widx, sample):
         counts, G, stats = plan.finalize()
         H = counts.cpu().numpy().view(np.uint64).copy()
         G = G.cpu().numpy()
+        c2all, g2all = plan.finalize_g2()
+        c2all = c2all.cpu().numpy().view(np.uint64).copy()
+        g2all = g2all.cpu().numpy()
+        T_r, _ = oracle_lib.thresholds(w.box, w.r_max, w.n_r, w.n_t)
         # per-frame histograms from the same plan; sampled ones against the oracle
         Hsum = np.zeros_like(H)
+        c2sum = np.zeros_like(c2all)
         pairs = 0
         for f in range(w.n_frames):
             plan.reset()
             plan.accumulate_frame(d_pos[f])
             cf, _, sf = plan.finalize(want_g3=False)
             Hf = cf.cpu().numpy().view(np.uint64)
+            c2f = plan.finalize_g2()[0].cpu().numpy().view(np.uint64)
             Hsum += Hf
+            c2sum += c2f
             pairs += sf[1]
             if f in sample:
                 Ho, so = oracle_frames(oracle_lib, w, [ms[f]])
                 assert np.array_equal(Hf, Ho), f"frame {f}"
                 assert sf == so
+                if f == sample[0]:
+                    assert np.array_equal(c2f, oracle_lib.g2_frame(ms[f], T_r)), f"g2, frame {f}"
+    assert np.array_equal(c2all, c2sum)
+    assert np.allclose(g2all, oracle_lib.g2_normalise(c2all, w.r_max, w.n_frames, w.n, w.box),
+                       rtol=G3_RTOL, atol=0)
+    if w.kind == "uniform":
+        z2 = (g2all / (1.0 - 1.0 / w.n) - 1.0) * np.sqrt(c2all.astype(np.float64) / 2.0)
+        assert np.abs(z2[4:]).max() < 6.0
     assert stats[0] == w.n_frames and stats[2] == 0
     assert np.array_equal(H, Hsum)                       # additivity over frames and batches
     assert stats[1] == pairs == int(H.sum())             # sum_i k_i (k_i - 1), overflow = 0

@@ -30,7 +30,9 @@ def run_gpu(g3, pos, box, r_max, n_r, n_t, **opts):
         d = torch.from_numpy(pos).cuda()
         plan.accumulate_frames(d)
         counts, g3v, stats = plan.finalize()
-        info = {"kernel": plan.info(g3.G3_INFO_KERNEL), "launches": plan.info(g3.G3_INFO_KERNEL_LAUNCHES)}
+        c2, g2 = plan.finalize_g2()
+        info = {"kernel": plan.info(g3.G3_INFO_KERNEL), "launches": plan.info(g3.G3_INFO_KERNEL_LAUNCHES),
+                "counts2": c2.cpu().numpy().view(np.uint64), "g2": g2.cpu().numpy()}
         return counts.cpu().numpy().view(np.uint64), g3v.cpu().numpy(), stats, info
 
 
@@ -46,6 +48,20 @@ def check(oracle_lib, g3, pos, box, r_max, n_r, n_t, mode="cells", **opts):
     assert np.array_equal(nz, G != 0)
     assert np.allclose(G[nz], Go[nz], rtol=G3_RTOL, atol=0)
     assert info["launches"] > 0
+    # g2 from the same neighbour pass: counts bit-exact, g2 to 1e-12.
+    # The g2 oracle is a plain O(N^2) loop: all frames for small systems, the first otherwise.
+    n = pos3.shape[1]
+    T_r, _ = oracle_lib.thresholds(box, r_max, n_r, n_t)
+    if n <= 40000:
+        H2 = np.zeros(n_r, dtype=np.uint64)
+        for f in range(pos3.shape[0]):
+            oracle_lib.g2_frame(oracle_lib.quantise(pos3[f], box), T_r, H2)
+        assert np.array_equal(info["counts2"], H2)
+        g2o = oracle_lib.g2_normalise(H2, r_max, pos3.shape[0], n, box)
+        assert np.allclose(info["g2"], g2o, rtol=G3_RTOL, atol=0)
+    else:
+        H2, _, _, i1 = run_gpu(g3, pos3[:1], box, r_max, n_r, n_t, **opts)
+        assert np.array_equal(i1["counts2"], oracle_lib.g2_frame(oracle_lib.quantise(pos3[0], box), T_r))
     if "kernel" in opts and opts["kernel"] in (1, 2) and opts.get("expect_kernel", True):
         pass
     return H, stats, info
