@@ -305,6 +305,18 @@ def run_ours(args):
         "hbm_gbs_achieved_step": F * w.n * 24 / (ms_dev * 1e-3) / 1e9,
         "hbm_gbs_peak": pk.get("hbm_gbs"),
     }
+    # the two candidate ceilings measured live on this GPU (g3_microbench): the
+    # shared-atomic rate for random slots of a tile as large as the kernel's, and the issue rate
+    atomic_rate = g3.microbench(0, min(plan.info(g3.G3_INFO_TILE_BINS), 56000), 1 << 15)
+    issue_rate = g3.microbench(1, 0, 1 << 18)
+    roofline.update({
+        "shared_atomic_per_s_measured": atomic_rate,
+        "frac_of_shared_atomic_ceiling": roofline["kernel_triplets_per_s"] / atomic_rate,
+        "issue_tinstr_per_s_measured": issue_rate / 1e12,
+        "binding_ceiling_triplets_per_s": min(atomic_rate, issue_rate / ALGO_INSTR_PER_TRIPLET),
+        "frac_of_binding_ceiling": roofline["kernel_triplets_per_s"]
+                                   / min(atomic_rate, issue_rate / ALGO_INSTR_PER_TRIPLET),
+    })
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu, _, _, _ = cpu_baseline_leg(w, args.cpu_budget)

@@ -23,7 +23,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_finalize_g2", "g3_normalize", "g3_bin_volumes", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -62,6 +62,7 @@ def load() -> C.CDLL:
     lib.g3_finalize_g2.argtypes = [vp, vp, vp, vp]
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
+    lib.g3_microbench.argtypes = [i32, i64, i64, C.POINTER(f64), vp]
     lib.g3_plan_reset.argtypes = [vp, vp]
     lib.g3_plan_destroy.argtypes = [vp]
     lib.g3_plan_destroy.restype = None
@@ -89,6 +90,14 @@ def _stream_ptr(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return int(stream.cuda_stream)
+
+
+def microbench(which: int, slots: int = 50776, iters: int = 1 << 14, stream=None) -> float:
+    """g3_microbench: 0 = shared-atomic increments/s (random slots), 1 = FP32 thread instr/s."""
+    rate = C.c_double()
+    _check(load().g3_microbench(int(which), int(slots), int(iters), C.byref(rate), _stream_ptr(stream)),
+           "g3_microbench")
+    return float(rate.value)
 
 
 class Plan:

@@ -17,6 +17,7 @@
 
 #include "g3_cells.cuh"
 #include "g3_generic.cuh"
+#include "g3_microbench.cuh"
 #include "g3_plan.h"
 #include "g3_tiled.cuh"
 #include "g3_volumes.h"
@@ -479,6 +480,44 @@ int g3_finalize_host(g3_plan* p, uint64_t* h_counts, double* h_g3, uint64_t* h_s
     }
     if (d_g3) cudaFreeAsync(d_g3, st);
     return rc;
+}
+
+int g3_microbench(int32_t which, int64_t slots, int64_t iters, double* h_rate, void* stream) {
+    if (!h_rate || iters < 8 || iters > (int64_t(1) << 30) || which < 0 || which > 1) return G3_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0;
+    cudaDeviceProp prop;
+    G3_CUDA(cudaGetDevice(&dev));
+    G3_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return G3_ECUDA;
+    const int grid = prop.multiProcessorCount;
+    const int32_t it = (int32_t)((iters + 127) / 128 * 128);
+    unsigned int* d_sink = nullptr;
+    G3_CUDA(cudaMalloc(&d_sink, 16));
+    cudaEvent_t e0, e1;
+    G3_CUDA(cudaEventCreate(&e0));
+    G3_CUDA(cudaEventCreate(&e1));
+    int rc = G3_OK;
+    float ms = 0.f;
+    for (int rep = 0; rep < 2 && rc == G3_OK; ++rep) {          // first pass warms up
+        cudaEventRecord(e0, st);
+        if (which == 0) {
+            if (slots < 32 || slots * 4 > (int64_t)prop.sharedMemPerBlockOptin) { rc = G3_EINVAL; break; }
+            cudaFuncSetAttribute(mb_shared_atomic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(slots * 4));
+            mb_shared_atomic_kernel<<<grid, kMbThreads, (size_t)slots * 4, st>>>((int32_t)slots, it, d_sink);
+        } else {
+            mb_issue_kernel<<<grid, kMbThreads, 0, st>>>(it, 1.0f, reinterpret_cast<float*>(d_sink));
+        }
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = G3_ECUDA;
+        else cudaEventElapsedTime(&ms, e0, e1);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_sink);
+    if (rc != G3_OK) return rc;
+    // thread-level operations per second over the whole GPU (loop overhead not counted)
+    *h_rate = (double)grid * kMbThreads * (double)it / ((double)ms * 1e-3);
+    return G3_OK;
 }
 
 int g3_bin_volumes(const g3_plan* p, double* h_volumes) {
