@@ -76,7 +76,8 @@ typedef enum {
 
 /* Options for g3_plan_set_option (all optional; defaults are chosen for the B200). */
 typedef enum {
-    G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1)      */
+    G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1);
+                                default: max(16, 2^19 / n) capped at 256 and by memory       */
     G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
     G3_OPT_MAX_NEIGHBOURS = 3, /* per-centre neighbour capacity (0 = derive from density)    */
     G3_OPT_TRIPLET_WARPS = 5, /* warps per triplet-kernel CTA: 0 = auto, or 8, 12, .. 24  */

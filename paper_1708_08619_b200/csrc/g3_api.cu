@@ -104,6 +104,11 @@ int configure(g3_plan* p) {
     cap = std::max<int64_t>((cap + 31) / 32 * 32, 64);   // >= 64: the triplet kernel prefetches two chunks
     p->max_nb = (int32_t)cap;
 
+    if (p->batch_auto) {
+        // small frames are launch-bound: stage enough frames for ~2^19 centres per launch sequence
+        const int64_t want = ((int64_t(1) << 19) + p->n - 1) / p->n;
+        p->batch_frames = (int32_t)std::min<int64_t>(std::max<int64_t>(want, 16), 256);
+    }
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled
     if (p->kernel == 1) {
         size_t smem = generic_smem_bytes(p->bins.n_r, p->bins.n_t, p->max_nb, kGenericWarps);
@@ -287,7 +292,7 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
     switch (option) {
         case G3_OPT_BATCH_FRAMES:
             if (value < 1 || value > 4096) return G3_EINVAL;
-            p->batch_frames = (int32_t)value; break;
+            p->batch_frames = (int32_t)value; p->batch_auto = false; break;
         case G3_OPT_KERNEL:
             if (value < 0 || value > 2) return G3_EINVAL;
             p->kernel_opt = (int32_t)value; break;
@@ -317,8 +322,7 @@ int g3_plan_get_info(const g3_plan* cp, int32_t key, int64_t* value) {
                : p->timed_launches;
         return G3_OK;
     }
-    if (key != G3_INFO_KERNEL_LAUNCHES && key != G3_INFO_FRAMES_PENDING && key != G3_INFO_SM_COUNT &&
-        key != G3_INFO_BATCH_FRAMES) {
+    if (key != G3_INFO_KERNEL_LAUNCHES && key != G3_INFO_FRAMES_PENDING && key != G3_INFO_SM_COUNT) {
         int rc = configure(p);
         if (rc != G3_OK) return rc;
     }

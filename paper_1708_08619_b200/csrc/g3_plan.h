@@ -51,7 +51,8 @@ struct g3_plan {
     int smem_optin = 0;
 
     // options / derived
-    int32_t batch_frames = 16;
+    int32_t batch_frames = 16;               // frames per launch sequence (see batch_auto)
+    bool batch_auto = true;                  // derive batch_frames from n: >= 2^19 centres per launch
     int32_t kernel_opt = 0;                  // G3_OPT_KERNEL
     int32_t kernel = 1;                      // selected kernel
     int32_t ncell = 1;
