@@ -42,7 +42,7 @@ ALGO_INSTR_PER_TRIPLET = 12          # fixed algorithmic instruc
 SM_LANES = 128                       # 4 schedulers x 32 lanes, one warp instruction per cycle each
 # dram__bytes_read.sum + dram__bytes_write.sum of one tiled_triplet_kernel launch (16 frames of
 # config 4) from the ncu --set full capture summarised in profiles/r1_triplet_kernel.md
-NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH = 598.814464e6 + 8.376832e6
+NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH = 598.884864e6 + 6.587904e6
 NCU_TRIPLET_FRAMES_PER_LAUNCH = 16
 
 
@@ -68,7 +68,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
