@@ -408,6 +408,108 @@ void g3o_g2_normalise(const uint64_t *H2, int32_t n_r, double r_max, int64_t n_f
     }
 }
 
+/* ------------------------------------------------------------------------- */
+/* q_tet: the tetrahedral order parameter, Eq. 1:
+ *     q = 1 - (3/8) sum_{j<k} (cos psi_jk + 1/3)^2
+ * over the six pairs of the FOUR NEAREST neighbours j, k of atom i, psi_jk the angle between
+ * the bond vectors r_ij and r_ik; Algorithm 2: all minimum-image distances
+ * from i, sort, four nearest, Eq. 1, "Update histogram with qtet".
+ * Readings (T1-T4; the paper states none of these):
+ *  T1 nearest = smallest squared minimum-image distance on the integer grid; ties are broken by
+ *     the vector itself, (d2, dx, dy, dz) in lexicographic order, so the choice does not depend
+ *     on particle numbering;
+ *  T2 arithmetic in fp64, one rounding per operation, in exactly this order: n_j = sqrt(d2_j);
+ *     c = dot / (n_j * n_k) with the integer dot product converted exactly; t = c + 1/3;
+ *     acc += t * t over (1,2),(1,3),(1,4),(2,3),(2,4),(3,4) of the sorted four; q = 1 - 0.375 acc;
+ *  T3 histogram: n_q bins of width 4/n_q on [-3, 1]; bin = floor((q + 3) * (n_q / 4)), q = 1
+ *     goes to the last bin;
+ *  T4 an atom with a coincident neighbour among the four (d2 = 0: no bond direction) is skipped
+ *     and counted in stats[1]; stats[0] counts the atoms binned.
+ * Plain all-pairs loop (no cell list); H [n_q] and stats [2] are ADDED to.                  */
+typedef struct { uint64_t d2; int64_t x, y, z; } qt_nb;
+
+static int qt_less(const qt_nb *a, const qt_nb *b)
+{
+    if (a->d2 != b->d2) return a->d2 < b->d2;
+    if (a->x != b->x) return a->x < b->x;
+    if (a->y != b->y) return a->y < b->y;
+    return a->z < b->z;
+}
+
+/* q of one atom from its four nearest neighbours, sorted (reading T2); returns 0 if skipped (T4) */
+static int qt_value(const qt_nb *nb, double *q)
+{
+    double nrm[4];
+    for (int j = 0; j < 4; ++j) {
+        if (nb[j].d2 == 0) return 0;
+        nrm[j] = sqrt((double)nb[j].d2);
+    }
+    double acc = 0.0;
+    for (int j = 0; j < 3; ++j)
+        for (int k = j + 1; k < 4; ++k) {
+            int64_t dot = nb[j].x * nb[k].x + nb[j].y * nb[k].y + nb[j].z * nb[k].z;
+            double den = nrm[j] * nrm[k];
+            double c = (double)dot / den;
+            double t = c + 1.0 / 3.0;
+            double t2 = t * t;
+            acc = acc + t2;
+        }
+    double s = 0.375 * acc;
+    *q = 1.0 - s;
+    return 1;
+}
+
+/* q_out (may be NULL): q of every atom of this frame, NaN where skipped.                   */
+void g3o_qtet_frame(const int32_t *m, int64_t n, int32_t n_q, uint64_t *H, uint64_t *stats,
+                    double *q_out)
+{
+    double scale = (double)n_q / 4.0;
+    uint64_t binned = 0, skipped = 0;
+#pragma omp parallel reduction(+ : binned, skipped)
+    {
+        uint64_t *h = (uint64_t *)calloc((size_t)n_q, sizeof(uint64_t));
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i) {
+            qt_nb best[4];
+            int have = 0;
+            for (int64_t j = 0; j < n; ++j) {
+                if (j == i) continue;
+                qt_nb c;
+                c.x = wrap((int64_t)m[3 * j + 0] - m[3 * i + 0]);
+                c.y = wrap((int64_t)m[3 * j + 1] - m[3 * i + 1]);
+                c.z = wrap((int64_t)m[3 * j + 2] - m[3 * i + 2]);
+                c.d2 = (uint64_t)(c.x * c.x + c.y * c.y + c.z * c.z);
+                /* insertion into the sorted list of the four smallest (T1) */
+                int pos = have;
+                while (pos > 0 && qt_less(&c, &best[pos - 1])) --pos;
+                if (pos >= 4) continue;
+                int last = have < 4 ? have : 3;
+                for (int t = last; t > pos; --t) best[t] = best[t - 1];
+                best[pos] = c;
+                if (have < 4) ++have;
+            }
+            double q;
+            if (have < 4 || !qt_value(best, &q)) {
+                skipped += 1;
+                if (q_out) q_out[i] = NAN;
+                continue;
+            }
+            if (q_out) q_out[i] = q;
+            double pos = (q + 3.0) * scale;
+            int64_t b = (int64_t)floor(pos);
+            if (b < 0) b = 0;
+            if (b > n_q - 1) b = n_q - 1;
+            h[b] += 1;
+            binned += 1;
+        }
+#pragma omp critical
+        for (int32_t b = 0; b < n_q; ++b) H[b] += h[b];
+        free(h);
+    }
+    stats[0] += binned;
+    stats[1] += skipped;
+}
+
 int32_t g3o_num_threads(void)
 {
 #ifdef _OPENMP

@@ -45,6 +45,8 @@ def _load() -> C.CDLL:
         _lib.g3o_g2_frame.restype = None
         _lib.g3o_g2_normalise.argtypes = [u64p, C.c_int32, C.c_double, C.c_int64, C.c_int64, C.c_double, f64p]
         _lib.g3o_g2_normalise.restype = None
+        _lib.g3o_qtet_frame.argtypes = [i32p, C.c_int64, C.c_int32, u64p, u64p, f64p]
+        _lib.g3o_qtet_frame.restype = None
         _lib.g3o_num_threads.restype = C.c_int32
         for fn in (_lib.g3o_thresholds, _lib.g3o_quantise, _lib.g3o_accumulate, _lib.g3o_volumes,
                    _lib.g3o_normalise):
@@ -146,6 +148,20 @@ def g2_normalise(H2: np.ndarray, r_max: float, n_frames: int, n: int, box: float
     g2 = np.zeros(H2.size, dtype=np.float64)
     _load().g3o_g2_normalise(_p(H2, C.c_uint64), H2.size, r_max, n_frames, n, box, _p(g2, C.c_double))
     return g2
+
+
+def qtet_frame(m: np.ndarray, n_q: int, H: Optional[np.ndarray] = None,
+               stats: Optional[np.ndarray] = None, q_out: Optional[np.ndarray] = None):
+    """Add one frame's q_tet histogram (n_q bins on [-3, 1]) to H; stats = [binned, skipped];
+    q_out (fp64 [n], optional) receives the per-atom values (NaN where skipped)."""
+    m = np.ascontiguousarray(m, dtype=np.int32)
+    if H is None:
+        H = np.zeros(n_q, dtype=np.uint64)
+    if stats is None:
+        stats = np.zeros(2, dtype=np.uint64)
+    qp = _p(q_out, C.c_double) if q_out is not None else None
+    _load().g3o_qtet_frame(_p(m, C.c_int32), m.shape[0], n_q, _p(H, C.c_uint64), _p(stats, C.c_uint64), qp)
+    return H, stats
 
 
 class Oracle:
