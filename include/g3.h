@@ -81,6 +81,9 @@ typedef enum {
     G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
     G3_OPT_MAX_NEIGHBOURS = 3, /* per-centre neighbour capacity (0 = derive from density)    */
     G3_OPT_TRIPLET_WARPS = 5, /* warps per triplet-kernel CTA: 0 = auto, or 8, 12, .. 24  */
+    G3_OPT_QTET_BINS = 6,    /* > 0: also histogram the tetrahedral order parameter q_tet (Eq. 1,
+                                PAPER.md:201) of every atom into this many bins on [-3, 1] while
+                                frames are accumulated; 0 (default) = off; needs n >= 5      */
     G3_OPT_TIMING = 4         /* 1 = bracket the neighbour and triplet kernels with CUDA events
                                  on the caller's stream (read back with g3_plan_get_info)     */
 } g3_option;
@@ -171,6 +174,16 @@ G3_API int g3_finalize_host(g3_plan *p, uint64_t *h_counts, double *h_g3, uint64
  *              rho = n / box^3 (ideal gas -> (n-1)/n); may be NULL
  * Does not synchronise and does not reset.  sum(counts2) = sum_i k_i.                */
 G3_API int g3_finalize_g2(g3_plan *p, uint64_t *d_counts2, double *d_g2, void *stream);
+
+/* q_tet, the tetrahedral order parameter (Eq. 1; Algorithms 2-3),
+ * histogrammed on the same cell list when G3_OPT_QTET_BINS > 0 (readings T1-T4: four
+ * nearest neighbours by (d^2, dx, dy, dz); fp64 in a fixed operation order; bins of width
+ * 4/n_q on [-3, 1], q = 1 in the last bin; atoms with a coincident neighbour are skipped).
+ * Reduces all staged frames, then copies the histogram and SYNCHRONISES `stream`.
+ *   d_hist   device, uint64 [n_q]; may be NULL
+ *   h_stats  host, uint64[2] = { atoms binned, atoms skipped }; may be NULL
+ * Errors: G3_ESTATE if the option is off.                                                  */
+G3_API int g3_finalize_qtet(g3_plan *p, uint64_t *d_hist, uint64_t *h_stats, void *stream);
 
 /* Normalise externally merged counts (e.g. the sum over ranks of a frame-sharded
  * run; the paper's "split the trajectory, merge the results"):

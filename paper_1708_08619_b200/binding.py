@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libg3.so")
 
 G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
 G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING, G3_OPT_TRIPLET_WARPS = 1, 2, 3, 4, 5
+G3_OPT_QTET_BINS = 6
 (G3_INFO_KERNEL_LAUNCHES, G3_INFO_BATCH_FRAMES, G3_INFO_KERNEL, G3_INFO_CELLS_PER_EDGE,
  G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING,
  G3_INFO_TRIPLET_NS, G3_INFO_NEIGHBOUR_NS, G3_INFO_TIMED_LAUNCHES, G3_INFO_SLABS) = range(1, 13)
@@ -23,7 +24,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_finalize_g2", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -60,6 +61,7 @@ def load() -> C.CDLL:
     lib.g3_finalize.argtypes = [vp, vp, vp, vp, vp]
     lib.g3_finalize_host.argtypes = [vp, vp, vp, vp, vp]
     lib.g3_finalize_g2.argtypes = [vp, vp, vp, vp]
+    lib.g3_finalize_qtet.argtypes = [vp, vp, vp, vp]
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
     lib.g3_microbench.argtypes = [i32, i64, i64, C.POINTER(f64), vp]
@@ -106,7 +108,7 @@ class Plan:
     def __init__(self, n: int, box: float, r_max: float, n_r: int, n_t: Optional[int] = None, *,
                  batch_frames: Optional[int] = None, kernel: Optional[int] = None,
                  max_neighbours: Optional[int] = None, timing: bool = False,
-                 triplet_warps: Optional[int] = None):
+                 triplet_warps: Optional[int] = None, qtet_bins: Optional[int] = None):
         self._lib = load()
         self.n, self.box, self.r_max = int(n), float(box), float(r_max)
         self.n_r, self.n_t = int(n_r), int(n_r if n_t is None else n_t)
@@ -123,6 +125,9 @@ class Plan:
             self.set_option(G3_OPT_TIMING, 1)
         if triplet_warps is not None:
             self.set_option(G3_OPT_TRIPLET_WARPS, triplet_warps)
+        self.qtet_bins = int(qtet_bins or 0)
+        if self.qtet_bins:
+            self.set_option(G3_OPT_QTET_BINS, self.qtet_bins)
 
     # -- options / info -------------------------------------------------------------------
     def set_option(self, option: int, value: int) -> None:
@@ -193,6 +198,15 @@ class Plan:
         _check(self._lib.g3_finalize_g2(self._h, counts2.data_ptr(), g2.data_ptr(), _stream_ptr(stream)),
                "g3_finalize_g2")
         return counts2, g2
+
+    def finalize_qtet(self, stream=None):
+        """(q_tet histogram int64-viewed-as-uint64 [qtet_bins] device tensor, [binned, skipped])."""
+        import torch
+        hist = torch.empty(self.qtet_bins, dtype=torch.int64, device="cuda")
+        stats = (C.c_uint64 * 2)()
+        _check(self._lib.g3_finalize_qtet(self._h, hist.data_ptr(), stats, _stream_ptr(stream)),
+               "g3_finalize_qtet")
+        return hist, [int(v) for v in stats]
 
     def normalize(self, d_counts, frames: int, stream=None):
         import torch

@@ -19,6 +19,7 @@
 #include "g3_generic.cuh"
 #include "g3_microbench.cuh"
 #include "g3_plan.h"
+#include "g3_qtet.cuh"
 #include "g3_tiled.cuh"
 #include "g3_volumes.h"
 
@@ -39,6 +40,7 @@ using namespace g3;
 namespace {
 
 constexpr int kGenericWarps = 8;
+constexpr int kQtetWarps = 8;
 
 __global__ void __launch_bounds__(256)
 normalise_kernel(const unsigned long long* __restrict__ counts, const double* __restrict__ volumes,
@@ -66,6 +68,8 @@ void free_buffers(g3_plan* p) {
     cudaFree(p->d_cell_start); p->d_cell_start = nullptr;
     cudaFree(p->d_sorted); p->d_sorted = nullptr;
     cudaFree(p->d_h2d); p->d_h2d = nullptr;
+    cudaFree(p->d_qtet); p->d_qtet = nullptr;
+    cudaFree(p->d_qtet_stats); p->d_qtet_stats = nullptr;
     tiled_free(p);
     p->configured = false;
 }
@@ -127,6 +131,14 @@ int configure(g3_plan* p) {
     G3_CUDA(cudaMalloc(&p->d_cell_start, sizeof(int32_t) * B * (nc3 + 1)));
     G3_CUDA(cudaMalloc(&p->d_sorted, sizeof(int4) * B * n));
     G3_CUDA(cudaMemset(p->d_cell_count, 0, sizeof(int32_t) * B * nc3));
+    if (p->qtet_bins > 0) {
+        G3_CUDA(cudaMalloc(&p->d_qtet, sizeof(unsigned long long) * p->qtet_bins));
+        G3_CUDA(cudaMalloc(&p->d_qtet_stats, sizeof(unsigned long long) * 2));
+        G3_CUDA(cudaMemset(p->d_qtet, 0, sizeof(unsigned long long) * p->qtet_bins));
+        G3_CUDA(cudaMemset(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2));
+        G3_CUDA(cudaFuncSetAttribute(qtet_kernel<kQtetWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(sizeof(unsigned int) * p->qtet_bins)));
+    }
     p->configured = true;
     return G3_OK;
 }
@@ -157,6 +169,14 @@ int flush(g3_plan* p, cudaStream_t st) {
         if (rc != G3_OK) return rc;
     }
     G3_CUDA(cudaGetLastError());
+    if (p->qtet_bins > 0) {                                // q_tet on the same cell list (Eq. 1)
+        const unsigned long long cw = (unsigned long long)(kGrid / p->ncell);
+        QtParams qp{p->qtet_bins, (double)p->qtet_bins / 4.0, cw * cw, p->d_qtet, p->d_qtet_stats};
+        long long blocks = std::min<long long>((total + kQtetWarps - 1) / kQtetWarps, (long long)p->sm_count * 8);
+        qtet_kernel<kQtetWarps><<<(unsigned)blocks, kQtetWarps * 32, sizeof(unsigned int) * p->qtet_bins, st>>>(fb, qp);
+        p->launches += 1;
+        G3_CUDA(cudaGetLastError());
+    }
     p->pending = 0;
     return G3_OK;
 }
@@ -302,6 +322,9 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
         case G3_OPT_TRIPLET_WARPS:
             if (value != 0 && (value < 8 || value > 24 || value % 4 != 0)) return G3_EINVAL;
             p->tri_warps_opt = (int32_t)value; break;
+        case G3_OPT_QTET_BINS:
+            if (value < 0 || value > 8192 || (value > 0 && p->n < 5)) return G3_EINVAL;
+            p->qtet_bins = (int32_t)value; break;
         case G3_OPT_TIMING:
             if (value < 0 || value > 1) return G3_EINVAL;
             p->timing = (int32_t)value; return G3_OK;
@@ -469,6 +492,23 @@ int g3_finalize_g2(g3_plan* p, uint64_t* d_counts2, double* d_g2, void* stream) 
     return G3_OK;
 }
 
+int g3_finalize_qtet(g3_plan* p, uint64_t* d_hist, uint64_t* h_stats, void* stream) {
+    if (!p) return G3_EINVAL;
+    if (p->qtet_bins <= 0) return G3_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = configure(p);
+    if (rc != G3_OK) return rc;
+    rc = flush(p, st);
+    if (rc != G3_OK) return rc;
+    if (d_hist)
+        G3_CUDA(cudaMemcpyAsync(d_hist, p->d_qtet, sizeof(uint64_t) * p->qtet_bins, cudaMemcpyDeviceToDevice, st));
+    unsigned long long stats[2] = {0, 0};
+    G3_CUDA(cudaMemcpyAsync(stats, p->d_qtet_stats, sizeof(stats), cudaMemcpyDeviceToHost, st));
+    G3_CUDA(cudaStreamSynchronize(st));
+    if (h_stats) { h_stats[0] = stats[0]; h_stats[1] = stats[1]; }
+    return G3_OK;
+}
+
 int g3_finalize_host(g3_plan* p, uint64_t* h_counts, double* h_g3, uint64_t* h_stats, void* stream) {
     if (!p) return G3_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -536,6 +576,10 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     G3_CUDA(cudaMemsetAsync(p->d_counts, 0, sizeof(unsigned long long) * p->nbins, st));
     G3_CUDA(cudaMemsetAsync(p->d_stats, 0, sizeof(unsigned long long) * 4, st));
     G3_CUDA(cudaMemsetAsync(p->d_counts2, 0, sizeof(unsigned long long) * p->bins.n_r, st));
+    if (p->d_qtet) {
+        G3_CUDA(cudaMemsetAsync(p->d_qtet, 0, sizeof(unsigned long long) * p->qtet_bins, st));
+        G3_CUDA(cudaMemsetAsync(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2, st));
+    }
     if (p->configured && p->pending) {
         const size_t nc3 = (size_t)p->ncell * p->ncell * p->ncell;
         G3_CUDA(cudaMemsetAsync(p->d_cell_count, 0, sizeof(int32_t) * p->batch_frames * nc3, st));

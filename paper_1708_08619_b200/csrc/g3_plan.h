@@ -70,6 +70,9 @@ struct g3_plan {
     unsigned long long* d_stats = nullptr;   // [4]: pairs, overflow, capacity error, spare
     double* d_volumes = nullptr;             // [nbins]
     double* d_volumes2 = nullptr;            // [n_r] shell volumes for g2
+    int32_t qtet_bins = 0;                   // G3_OPT_QTET_BINS: 0 = q_tet off
+    unsigned long long* d_qtet = nullptr;    // [qtet_bins] histogram of q_tet on [-3, 1]
+    unsigned long long* d_qtet_stats = nullptr; // [2]: atoms binned, atoms skipped
     int4* d_staged = nullptr;                // [batch][n] quantised (x,y,z,cell) in input order
     int32_t* d_slot = nullptr;               // [batch][n] rank of the particle inside its cell
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]
