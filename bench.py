@@ -317,6 +317,25 @@ def run_ours(args):
         "frac_of_binding_ceiling": roofline["kernel_triplets_per_s"]
                                    / min(atomic_rate, issue_rate / ALGO_INSTR_PER_TRIPLET),
     })
+    # q_tet on the same cell list, timed as the EXTRA cost over the g3 path
+    # (same trajectory, a second plan with G3_OPT_QTET_BINS on; the difference of two device times)
+    qtet = None
+    try:
+        if world > 1:
+            raise RuntimeError("measured at --gpus 1 only")
+        with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, qtet_bins=200) as qplan:
+            def step_q():
+                qplan.reset()
+                qplan.accumulate_frames(d_pos)
+                qplan.finalize(want_g3=False)
+                return qplan.finalize_qtet()
+            step_q()
+            ms_q, (qh, qs), _, _ = timed(step_q, 2)
+            extra = max(ms_q - ms_dev, 1e-6)
+            qtet = {"atoms_binned_per_step": qs[0], "extra_ms_per_step": extra,
+                    "atoms_per_s_extra": qs[0] / (extra * 1e-3), "bins": 200}
+    except Exception as e:  # the g3 numbers above stay valid
+        qtet = {"error": str(e)}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu, _, _, _ = cpu_baseline_leg(w, args.cpu_budget)
@@ -340,6 +359,7 @@ def run_ours(args):
         "gpu_launches": launches * args.steps,
         "gpu_launches_per_step": launches,
         "roofline": roofline,
+        "qtet": qtet,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)

@@ -70,6 +70,8 @@ void free_buffers(g3_plan* p) {
     cudaFree(p->d_h2d); p->d_h2d = nullptr;
     cudaFree(p->d_qtet); p->d_qtet = nullptr;
     cudaFree(p->d_qtet_stats); p->d_qtet_stats = nullptr;
+    cudaFree(p->d_qtet_redo); p->d_qtet_redo = nullptr;
+    cudaFree(p->d_qtet_origin); p->d_qtet_origin = nullptr;
     tiled_free(p);
     p->configured = false;
 }
@@ -138,6 +140,27 @@ int configure(g3_plan* p) {
         G3_CUDA(cudaMemset(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2));
         G3_CUDA(cudaFuncSetAttribute(qtet_kernel<kQtetWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)(sizeof(unsigned int) * p->qtet_bins)));
+        G3_CUDA(cudaFuncSetAttribute(qtet_redo_kernel<kQtetWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(sizeof(unsigned int) * p->qtet_bins)));
+        if (p->ncell > 1 && B * n < (int64_t(1) << 31)) {   // fast path: 27 cells staged per CTA
+            p->qtet_stage_cap = tiled_stage_cap(p);
+            const size_t smem = qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins);
+            if (smem <= (size_t)p->smem_optin) {
+                G3_CUDA(cudaFuncSetAttribute(qtet_cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                G3_CUDA(cudaMalloc(&p->d_qtet_redo, sizeof(int32_t) * (size_t)(B * n + 1)));
+                const int32_t nc = p->ncell;
+                std::vector<int4> origin((size_t)nc3);
+                for (int32_t cx = 0; cx < nc; ++cx)
+                    for (int32_t cy = 0; cy < nc; ++cy)
+                        for (int32_t cz = 0; cz < nc; ++cz)
+                            origin[((size_t)cx * nc + cy) * nc + cz] =
+                                make_int4((int32_t)(((int64_t)(2 * cx + 1) << (kGridBits - 1)) / nc),
+                                          (int32_t)(((int64_t)(2 * cy + 1) << (kGridBits - 1)) / nc),
+                                          (int32_t)(((int64_t)(2 * cz + 1) << (kGridBits - 1)) / nc), 0);
+                G3_CUDA(cudaMalloc(&p->d_qtet_origin, sizeof(int4) * origin.size()));
+                G3_CUDA(cudaMemcpy(p->d_qtet_origin, origin.data(), sizeof(int4) * origin.size(), cudaMemcpyHostToDevice));
+            }
+        }
     }
     p->configured = true;
     return G3_OK;
@@ -171,10 +194,22 @@ int flush(g3_plan* p, cudaStream_t st) {
     G3_CUDA(cudaGetLastError());
     if (p->qtet_bins > 0) {                                // q_tet on the same cell list (Eq. 1)
         const unsigned long long cw = (unsigned long long)(kGrid / p->ncell);
-        QtParams qp{p->qtet_bins, (double)p->qtet_bins / 4.0, cw * cw, p->d_qtet, p->d_qtet_stats};
-        long long blocks = std::min<long long>((total + kQtetWarps - 1) / kQtetWarps, (long long)p->sm_count * 8);
-        qtet_kernel<kQtetWarps><<<(unsigned)blocks, kQtetWarps * 32, sizeof(unsigned int) * p->qtet_bins, st>>>(fb, qp);
-        p->launches += 1;
+        QtParams qp{p->qtet_bins, (double)p->qtet_bins / 4.0, cw * cw, p->d_qtet, p->d_qtet_stats,
+                    p->qtet_stage_cap, p->d_qtet_origin, p->d_qtet_redo, 0};
+        const size_t hist_smem = sizeof(unsigned int) * p->qtet_bins;
+        if (p->d_qtet_redo) {
+            G3_CUDA(cudaMemsetAsync(p->d_qtet_redo, 0, sizeof(int32_t), st));
+            const long long items = (long long)nc3 * F;
+            qtet_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->sm_count * 8), kQtCellWarps * 32,
+                               qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins), st>>>(fb, qp);
+            qp.use_redo = 1;                               // the few atoms the fast path could not decide
+            qtet_redo_kernel<kQtetWarps><<<(unsigned)p->sm_count * 2, kQtetWarps * 32, hist_smem, st>>>(fb, qp);
+            p->launches += 2;
+        } else {
+            long long blocks = std::min<long long>((total + kQtetWarps - 1) / kQtetWarps, (long long)p->sm_count * 8);
+            qtet_kernel<kQtetWarps><<<(unsigned)blocks, kQtetWarps * 32, hist_smem, st>>>(fb, qp);
+            p->launches += 1;
+        }
         G3_CUDA(cudaGetLastError());
     }
     p->pending = 0;

@@ -73,6 +73,9 @@ struct g3_plan {
     int32_t qtet_bins = 0;                   // G3_OPT_QTET_BINS: 0 = q_tet off
     unsigned long long* d_qtet = nullptr;    // [qtet_bins] histogram of q_tet on [-3, 1]
     unsigned long long* d_qtet_stats = nullptr; // [2]: atoms binned, atoms skipped
+    int32_t* d_qtet_redo = nullptr;          // [1 + batch * n]: atoms handed to the exact routine
+    int4* d_qtet_origin = nullptr;           // [ncell3] cell centres on the grid
+    int32_t qtet_stage_cap = 0;
     int4* d_staged = nullptr;                // [batch][n] quantised (x,y,z,cell) in input order
     int32_t* d_slot = nullptr;               // [batch][n] rank of the particle inside its cell
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]

@@ -10,9 +10,21 @@
 // fourth distance is below that width; otherwise (sparse frames) the atom is redone against all
 // particles.  Lane 0 evaluates Eq. 1 in fp64 with one rounding per operation in the fixed order
 // of reading T2, so the bin of q is decided by IEEE fp64 arithmetic alone.
+//
+// Two kernels.  qtet_cell_kernel is the fast one: a CTA stages the 27 cells once in shared memory
+// as fp32 coordinates relative to the cell centre (exact integers, as in g3_neighbour.cuh) and a
+// warp per atom (1) scans them in fp32, each lane keeping its four smallest d2 (a min/max
+// insertion network, no divergence), (2) takes the warp's fourth smallest value tau with four
+// REDUX.MIN rounds, (3) rescans and ballot-compacts the candidates with d2 <= tau (1 + 2^-20) --
+// a superset of the true four nearest, because fp32 d2 is within 2^-22 of the exact integer --
+// and (4) orders those few by the exact 64-bit key.  qtet_kernel is the plain exact routine
+// (64-bit keys straight from global memory); it serves degenerate cell grids and the atoms the
+// fast kernel hands over (fourth neighbour not provably inside the 27 cells, crowded stage, or
+// more than 32 candidates inside the tolerance).
 #pragma once
 
 #include "g3_generic.cuh"
+#include "g3_neighbour.cuh"
 #include "g3_plan.h"
 
 namespace g3 {
@@ -23,6 +35,10 @@ struct QtParams {
     unsigned long long guarantee2;        // (cell width)^2: below it the 27-cell search is exact
     unsigned long long* hist;             // [n_q]
     unsigned long long* stats;            // [2]: atoms binned, atoms skipped
+    int32_t stage_cap;                    // qtet_cell_kernel: staged candidates per CTA
+    const int4* cell_origin;              // [ncell3] grid coordinates of the cell centres
+    int32_t* redo;                        // [frames * n + 1]: count, then atoms handed to qtet_kernel
+    int32_t use_redo;                     // qtet_kernel: 1 = process the redo list, 0 = every atom
 };
 
 struct QtKey {
@@ -78,6 +94,52 @@ __device__ __forceinline__ void qt_merge(QtKey (&top)[4], int lane, QtKey (&best
     }
 }
 
+// Eq. 1 for one atom from its four nearest neighbours `best` (sorted by key), evaluated by one
+// lane in fp64, one rounding per operation, in the order of reading T2; then the bin (T3, T4).
+__device__ __forceinline__ void qt_finish(const QtKey (&best)[4], const QtParams& qp, unsigned int* hist_s,
+                                          unsigned long long& binned, unsigned long long& skipped) {
+    if (best[3].hi == ~0ull || best[0].hi == 0ull) { skipped += 1; return; }       // T4
+    double nrm[4];
+    long long vx[4], vy[4], vz[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        nrm[j] = __dsqrt_rn((double)best[j].hi);
+        vx[j] = (long long)(best[j].lo >> 40) - 524288;
+        vy[j] = (long long)((best[j].lo >> 20) & 0xFFFFF) - 524288;
+        vz[j] = (long long)(best[j].lo & 0xFFFFF) - 524288;
+    }
+    double acc = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int k = j + 1; k < 4; ++k) {
+            const long long dot = vx[j] * vx[k] + vy[j] * vy[k] + vz[j] * vz[k];
+            const double den = __dmul_rn(nrm[j], nrm[k]);
+            const double c = __ddiv_rn((double)dot, den);
+            const double t = __dadd_rn(c, 1.0 / 3.0);
+            acc = __dadd_rn(acc, __dmul_rn(t, t));
+        }
+    const double q = __dsub_rn(1.0, __dmul_rn(0.375, acc));
+    long long b = (long long)floor(__dmul_rn(__dadd_rn(q, 3.0), qp.scale));
+    b = b < 0 ? 0 : (b > qp.n_q - 1 ? qp.n_q - 1 : b);
+    atomicAdd(hist_s + b, 1u);
+    binned += 1;
+}
+
+__device__ __forceinline__ void qt_flush(const QtParams& qp, const unsigned int* hist_s,
+                                         unsigned long long binned, unsigned long long skipped) {
+    __syncthreads();
+    for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) {
+        const unsigned int v = hist_s[i];
+        if (v) atomicAdd(qp.hist + i, (unsigned long long)v);
+    }
+    if (binned) atomicAdd(qp.stats + 0, binned);
+    if (skipped) atomicAdd(qp.stats + 1, skipped);
+}
+
+// Plain exact routine: 64-bit keys straight from global memory, warp per atom.  use_redo = 0:
+// every atom of the batch (27 cells first, all particles if the fourth neighbour is not provably
+// inside them); use_redo = 1: only the atoms listed by qtet_cell_kernel, against all particles.
 template <int kWarps>
 __global__ void __launch_bounds__(kWarps * 32)
 qtet_kernel(FrameBatch fb, QtParams qp) {
@@ -85,66 +147,254 @@ qtet_kernel(FrameBatch fb, QtParams qp) {
     for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) qt_hist[i] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long long total = (long long)fb.n_frames * fb.n;
+    const long long total = qp.use_redo ? (long long)qp.redo[0] : (long long)fb.n_frames * fb.n;
     unsigned long long binned = 0, skipped = 0;
-    for (long long g = (long long)blockIdx.x * kWarps + wid; g < total; g += (long long)gridDim.x * kWarps) {
+    for (long long it = (long long)blockIdx.x * kWarps + wid; it < total; it += (long long)gridDim.x * kWarps) {
+        const long long g = qp.use_redo ? (long long)qp.redo[1 + it] : it;
         const int32_t f = (int32_t)(g / fb.n);
         const int32_t s = (int32_t)(g - (long long)f * fb.n);
         const int4* __restrict__ sorted = fb.sorted + (long long)f * fb.n;
         const int32_t* __restrict__ start = fb.cell_start + (long long)f * (fb.ncell3 + 1);
         const int4 me = sorted[s];
         QtKey top[4], best[4];
+        bool exact = false;
+        if (!qp.use_redo) {
 #pragma unroll
-        for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
-        const int32_t n_ranges = CandidateRanges::count(fb.ncell);
-        for (int32_t r = 0; r < n_ranges; ++r) {
-            int32_t begin, end;
-            CandidateRanges::get(r, me.w, fb.ncell, fb.n, start, begin, end);
-            qt_scan(sorted, begin, end, s, me, lane, top);
+            for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
+            const int32_t n_ranges = CandidateRanges::count(fb.ncell);
+            for (int32_t r = 0; r < n_ranges; ++r) {
+                int32_t begin, end;
+                CandidateRanges::get(r, me.w, fb.ncell, fb.n, start, begin, end);
+                qt_scan(sorted, begin, end, s, me, lane, top);
+            }
+            qt_merge(top, lane, best);
+            exact = fb.ncell == 1 || best[3].hi < qp.guarantee2;
         }
-        qt_merge(top, lane, best);
-        if (fb.ncell != 1 && best[3].hi >= qp.guarantee2) {      // sparse neighbourhood: all particles
+        if (!exact) {                                            // all particles of the frame
 #pragma unroll
             for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
             qt_scan(sorted, 0, fb.n, s, me, lane, top);
             qt_merge(top, lane, best);
         }
-        if (lane != 0) continue;
-        // Eq. 1 in fp64, one rounding per operation, in the order of reading T2
-        if (best[3].hi == ~0ull || best[0].hi == 0ull) { skipped += 1; continue; }   // T4
-        double nrm[4];
-        long long vx[4], vy[4], vz[4];
+        if (lane == 0) qt_finish(best, qp, qt_hist, binned, skipped);
+    }
+    qt_flush(qp, qt_hist, binned, skipped);
+}
+
+// The atoms qtet_cell_kernel could not decide, against ALL particles of their frame: a whole CTA
+// per atom (the list is short, so one warp per atom would leave the GPU idle behind a few long
+// scans).  Every warp scans a slice, the per-warp results are merged through shared memory.
+template <int kWarps>
+__global__ void __launch_bounds__(kWarps * 32)
+qtet_redo_kernel(FrameBatch fb, QtParams qp) {
+    extern __shared__ unsigned int qt_hist[];
+    __shared__ ulonglong2 part[kWarps * 4];
+    static_assert(kWarps * 4 <= 32, "one warp merges the partial results");
+    for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) qt_hist[i] = 0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t total = qp.redo[0];
+    unsigned long long binned = 0, skipped = 0;
+    for (int32_t it = blockIdx.x; it < total; it += gridDim.x) {
+        const long long g = qp.redo[1 + it];
+        const int32_t f = (int32_t)(g / fb.n);
+        const int32_t s = (int32_t)(g - (long long)f * fb.n);
+        const int4* __restrict__ sorted = fb.sorted + (long long)f * fb.n;
+        const int4 me = sorted[s];
+        QtKey top[4], best[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            nrm[j] = __dsqrt_rn((double)best[j].hi);
-            vx[j] = (long long)(best[j].lo >> 40) - 524288;
-            vy[j] = (long long)((best[j].lo >> 20) & 0xFFFFF) - 524288;
-            vz[j] = (long long)(best[j].lo & 0xFFFFF) - 524288;
+        for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
+        for (int32_t p0 = wid * 32; p0 < fb.n; p0 += kWarps * 32)
+            qt_scan(sorted, p0, min(p0 + 32, fb.n), s, me, lane, top);
+        qt_merge(top, lane, best);
+        __syncthreads();                                   // `part` of the previous atom is free
+        if (lane == 0) {
+#pragma unroll
+            for (int t = 0; t < 4; ++t) part[wid * 4 + t] = make_ulonglong2(best[t].hi, best[t].lo);
         }
-        double acc = 0.0;
+        __syncthreads();
+        if (wid == 0) {
 #pragma unroll
-        for (int j = 0; j < 3; ++j)
+            for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
+            if (lane < kWarps * 4) { top[0].hi = part[lane].x; top[0].lo = part[lane].y; }
+            qt_merge(top, lane, best);
+            if (lane == 0) qt_finish(best, qp, qt_hist, binned, skipped);
+        }
+    }
+    qt_flush(qp, qt_hist, binned, skipped);
+}
+
+constexpr int kQtCellWarps = 4;
+constexpr int kQtSlots = 64;                    // atoms of one cell whose result is kept in shared memory
+
+// sorted insertion of x into the ascending four a[0..3] (the largest of the five drops out)
+__device__ __forceinline__ void qt_insert4(uint32_t (&a)[4], uint32_t x) {
+    uint32_t lo;
+    lo = min(a[0], x); x = max(a[0], x); a[0] = lo;
+    lo = min(a[1], x); x = max(a[1], x); a[1] = lo;
+    lo = min(a[2], x); x = max(a[2], x); a[2] = lo;
+    a[3] = min(a[3], x);
+}
+
+// Fast path (see the file header).  Persistent: a CTA strides over (cell, frame) items.  The fp32
+// d2 of a candidate is kept as its bit pattern (order-preserving for non-negative floats) with the
+// scan iteration in the low 5 bits, so a lane can fetch its kept candidates again; the 2^-18
+// perturbation this causes is covered by the 2^-16 tolerance of step (3).
+__global__ void __launch_bounds__(kQtCellWarps * 32)
+qtet_cell_kernel(FrameBatch fb, QtParams qp) {
+    extern __shared__ __align__(16) unsigned char qt_smem[];
+    float4* stage = reinterpret_cast<float4*>(qt_smem);
+    ulonglong2* scratch_all = reinterpret_cast<ulonglong2*>(stage + qp.stage_cap);      // [warps][32] keys
+    ulonglong2* best_s = scratch_all + kQtCellWarps * 32;                              // [kQtSlots][4]
+    unsigned int* hist_s = reinterpret_cast<unsigned int*>(best_s + kQtSlots * 4);
+    __shared__ int32_t range_begin[kMaxRanges], range_prefix[kMaxRanges + 1];
+    __shared__ int32_t own_base_s, cell_range[2];
+    __shared__ int32_t decided_s[kQtSlots];
+
+    for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) hist_s[i] = 0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    ulonglong2* scratch = scratch_all + wid * 32;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    constexpr uint32_t kInfBits = 0x7F000000u;             // 1.7e38 as fp32 bits
+    unsigned long long binned = 0, skipped = 0;
+    const long long n_items = (long long)fb.ncell3 * fb.n_frames;
+    const int32_t n_ranges = CandidateRanges::count(fb.ncell);
+
+    for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int32_t f = (int32_t)(item / fb.ncell3), cell = (int32_t)(item - (long long)f * fb.ncell3);
+        const int4* __restrict__ sorted = fb.sorted + (long long)f * fb.n;
+        const int32_t* __restrict__ start = fb.cell_start + (long long)f * (fb.ncell3 + 1);
+        __syncthreads();                                   // the previous item's shared state is free
+        if (wid == 0) {
+            const int32_t c_begin = __ldg(start + cell), c_end = __ldg(start + cell + 1);
+            int32_t b = 0, e = 0;
+            if (lane < n_ranges) CandidateRanges::get(lane, cell, fb.ncell, fb.n, start, b, e);
+            const int32_t len = e - b;
+            int32_t incl = len;
 #pragma unroll
-            for (int k = j + 1; k < 4; ++k) {
-                const long long dot = vx[j] * vx[k] + vy[j] * vy[k] + vz[j] * vz[k];
-                const double den = __dmul_rn(nrm[j], nrm[k]);
-                const double c = __ddiv_rn((double)dot, den);
-                const double t = __dadd_rn(c, 1.0 / 3.0);
-                acc = __dadd_rn(acc, __dmul_rn(t, t));
+            for (int d = 1; d < 32; d <<= 1) {
+                const int32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
             }
-        const double q = __dsub_rn(1.0, __dmul_rn(0.375, acc));
-        long long b = (long long)floor(__dmul_rn(__dadd_rn(q, 3.0), qp.scale));
-        b = b < 0 ? 0 : (b > qp.n_q - 1 ? qp.n_q - 1 : b);
-        atomicAdd(qt_hist + b, 1u);
-        binned += 1;
+            if (lane < n_ranges) { range_begin[lane] = b; range_prefix[lane] = incl - len; }
+            if (lane == n_ranges - 1) range_prefix[n_ranges] = incl;
+            if (lane < n_ranges && b <= c_begin && c_begin < e) own_base_s = incl - len + (c_begin - b);
+            if (lane == 0) { cell_range[0] = c_begin; cell_range[1] = c_end; }
+        }
+        __syncthreads();
+        const int32_t c_begin = cell_range[0], c_end = cell_range[1];
+        if (c_begin == c_end) continue;                    // empty cell (uniform over the CTA)
+        const int32_t n_stage = range_prefix[n_ranges];
+        const int32_t n_pad = (n_stage + 31) & ~31;
+        const bool staged = n_pad <= qp.stage_cap && n_pad <= 1024;      // iteration index fits 5 bits
+        if (staged) {
+            const int4 o = __ldg(qp.cell_origin + cell);
+            for (int32_t r = wid; r < n_ranges; r += kQtCellWarps) {
+                const int32_t b = range_begin[r], dst = range_prefix[r], len = range_prefix[r + 1] - dst;
+                for (int32_t i = lane; i < len; i += 32) {
+                    const int4 c = sorted[b + i];
+                    stage[dst + i] = make_float4((float)wrap_component(c.x - o.x), (float)wrap_component(c.y - o.y),
+                                                 (float)wrap_component(c.z - o.z), 0.f);
+                }
+            }
+            for (int32_t i = n_stage + threadIdx.x; i < n_pad; i += blockDim.x)
+                stage[i] = make_float4(kFarAway, 0.f, 0.f, 0.f);
+        }
+        __syncthreads();
+        const int32_t own_base = own_base_s;
+        for (int32_t s = c_begin + wid; s < c_end; s += kQtCellWarps) {
+            const int32_t slot = s - c_begin;
+            bool decided = false;
+            if (staged && slot < kQtSlots) {
+                const int32_t own = own_base + slot;
+                const float4 p = stage[own];
+                const int32_t own_it = own >> 5;
+                const bool own_lane = lane == (own & 31);
+                const float4* __restrict__ sp = stage + lane;
+                // (1) per-lane four smallest fp32 d2 (bit patterns tagged with the iteration)
+                uint32_t a[4] = {kInfBits, kInfBits, kInfBits, kInfBits};
+                const int32_t n_it = n_pad >> 5;
+#pragma unroll 2
+                for (int32_t it = 0; it < n_it; ++it) {
+                    const float4 c = sp[it << 5];
+                    const float dx = c.x - p.x, dy = c.y - p.y, dz = c.z - p.z;
+                    const float d2f = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    const uint32_t bits = (__float_as_uint(d2f) & ~31u) | (uint32_t)it;
+                    qt_insert4(a, own_lane && it == own_it ? kInfBits : bits);
+                }
+                // (2) the warp's fourth smallest
+                uint32_t h[4] = {a[0], a[1], a[2], a[3]};
+                uint32_t tau_bits = 0;
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    tau_bits = __reduce_min_sync(0xffffffffu, h[0]);
+                    const unsigned who = __ballot_sync(0xffffffffu, h[0] == tau_bits);
+                    if (lane == __ffs(who) - 1) { h[0] = h[1]; h[1] = h[2]; h[2] = h[3]; h[3] = kInfBits; }
+                }
+                if (tau_bits < 0x60000000u) {              // at least four real candidates (sentinels: 9e36)
+                    // (3) candidates within the fp32 tolerance of tau: exact 64-bit keys to scratch
+                    const float cut = __fmul_ru(__uint_as_float(tau_bits | 31u), 1.0f + 1.52587890625e-5f);
+                    const uint32_t cut_bits = __float_as_uint(cut) | 31u;
+                    bool lost = a[3] <= cut_bits;          // a fifth candidate of this lane may have dropped out
+                    int32_t count = 0;
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) {
+                        const bool acc = a[t] <= cut_bits;
+                        const unsigned mask = __ballot_sync(0xffffffffu, acc);
+                        const int32_t pos = count + __popc(mask & lt_mask);
+                        if (acc && pos < 32) {
+                            const float4 c = sp[(a[t] & 31u) << 5];
+                            const long long X = (long long)(c.x - p.x), Y = (long long)(c.y - p.y),
+                                            Z = (long long)(c.z - p.z);
+                            scratch[pos] = make_ulonglong2(
+                                (unsigned long long)(X * X + Y * Y + Z * Z),
+                                ((unsigned long long)(X + 524288) << 40) | ((unsigned long long)(Y + 524288) << 20) |
+                                    (unsigned long long)(Z + 524288));
+                        }
+                        count += __popc(mask);
+                    }
+                    lost = __any_sync(0xffffffffu, lost) || count > 32;
+                    __syncwarp();
+                    if (!lost) {
+                        // (4) rank of every candidate by the exact key (ties by scratch position)
+                        ulonglong2 my = make_ulonglong2(~0ull, ~0ull);
+                        if (lane < count) my = scratch[lane];
+                        int32_t rank = 0;
+                        for (int32_t e = 0; e < count; ++e) {
+                            const ulonglong2 k = scratch[e];
+                            rank += (k.x < my.x || (k.x == my.x && (k.y < my.y || (k.y == my.y && e < lane)))) ? 1 : 0;
+                        }
+                        const bool mine = lane < count && rank < 4;
+                        if (mine) best_s[slot * 4 + rank] = my;
+                        decided = __any_sync(0xffffffffu, mine && rank == 3 && my.x < qp.guarantee2);
+                    }
+                    __syncwarp();
+                }
+            }
+            if (lane == 0) {
+                if (slot < kQtSlots) decided_s[slot] = decided ? 1 : 0;
+                if (!decided) {                            // hand the atom to the exact routine
+                    const int32_t idx = atomicAdd(qp.redo, 1);
+                    qp.redo[1 + idx] = (int32_t)((long long)f * fb.n + s);
+                }
+            }
+        }
+        __syncthreads();
+        // Eq. 1: one thread per decided atom of the cell
+        if ((int32_t)threadIdx.x < min(c_end - c_begin, kQtSlots) && decided_s[threadIdx.x]) {
+            QtKey best[4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                const ulonglong2 k = best_s[threadIdx.x * 4 + t];
+                best[t].hi = k.x; best[t].lo = k.y;
+            }
+            qt_finish(best, qp, hist_s, binned, skipped);
+        }
     }
-    __syncthreads();
-    for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) {
-        const unsigned int v = qt_hist[i];
-        if (v) atomicAdd(qp.hist + i, (unsigned long long)v);
-    }
-    if (binned) atomicAdd(qp.stats + 0, binned);
-    if (skipped) atomicAdd(qp.stats + 1, skipped);
+    qt_flush(qp, hist_s, binned, skipped);
+}
+
+inline size_t qtet_cell_smem_bytes(int32_t stage_cap, int32_t n_q) {
+    return (size_t)stage_cap * 16 + (size_t)kQtCellWarps * 32 * 16 + (size_t)kQtSlots * 4 * 16 + (size_t)n_q * 4;
 }
 
 }  // namespace g3
