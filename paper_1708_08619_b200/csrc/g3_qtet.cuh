@@ -2,25 +2,25 @@
 // NEXT-3): Eq. 1, Algorithm 3 CUDA_qtet, which runs loops 3-5
 // of Algorithm 2 for one atom per thread and updates the histogram with atomicAdd.
 //
-// Here: one warp per atom.  The lanes scan the 27 cells around the atom (or the whole frame when
-// the cell grid is degenerate), each lane keeping its own four smallest keys
-//     key = (d2, dx, dy, dz)  in lexicographic order            (reading T1)
-// in registers; four rounds of a warp-wide minimum then give the four nearest neighbours.  Every
-// particle outside the 27 cells is more than one cell width away, so the result is exact when the
-// fourth distance is below that width; otherwise (sparse frames) the atom is redone against all
-// particles.  Lane 0 evaluates Eq. 1 in fp64 with one rounding per operation in the fixed order
-// of reading T2, so the bin of q is decided by IEEE fp64 arithmetic alone.
-//
-// Two kernels.  qtet_cell_kernel is the fast one: a CTA stages the 27 cells once in shared memory
-// as fp32 coordinates relative to the cell centre (exact integers, as in g3_neighbour.cuh) and a
-// warp per atom (1) scans them in fp32, each lane keeping its four smallest d2 (a min/max
-// insertion network, no divergence), (2) takes the warp's fourth smallest value tau with four
-// REDUX.MIN rounds, (3) rescans and ballot-compacts the candidates with d2 <= tau (1 + 2^-20) --
-// a superset of the true four nearest, because fp32 d2 is within 2^-22 of the exact integer --
-// and (4) orders those few by the exact 64-bit key.  qtet_kernel is the plain exact routine
-// (64-bit keys straight from global memory); it serves degenerate cell grids and the atoms the
-// fast kernel hands over (fourth neighbour not provably inside the 27 cells, crowded stage, or
-// more than 32 candidates inside the tolerance).
+// Three kernels.
+//  qtet_cell_kernel, the fast one: a CTA stages the 27 cells once in shared memory as fp32
+//   coordinates relative to the cell centre (exact integers, as in g3_neighbour.cuh) and a warp per
+//   atom (1) scans them in fp32, each lane keeping its four smallest d2 as bit patterns tagged with
+//   the scan iteration (a min/max insertion network, no divergence), (2) takes the warp's fourth
+//   smallest value tau with four REDUX.MIN rounds, (3) fetches again the kept candidates with
+//   d2 <= tau (1 + 2^-16) -- a superset of the true four nearest, because the tagged fp32 d2 is
+//   within 2^-18 + 2^-22 of the exact integer -- and writes their exact 64-bit keys
+//       key = (d2, dx, dy, dz)  in lexicographic order            (reading T1)
+//   to a per-warp list, (4) ranks those few by the exact key.  Every particle outside the 27 cells
+//   is more than one cell width away, so the result is exact when the fourth distance is below
+//   that width.  One THREAD per atom of the cell then evaluates Eq. 1 in fp64 with one rounding
+//   per operation in the fixed order of reading T2, so the bin of q is decided by IEEE
+//   fp64 arithmetic alone.
+//  qtet_redo_kernel: the atoms the fast kernel hands over (fourth neighbour not provably inside
+//   the 27 cells, a lane that may have dropped a fifth candidate inside the tolerance, crowded
+//   stage, more than 64 atoms in the cell), a whole CTA per atom against all particles.
+//  qtet_kernel: the plain exact routine (64-bit keys straight from global memory, warp per atom)
+//   for degenerate cell grids.
 #pragma once
 
 #include "g3_generic.cuh"
