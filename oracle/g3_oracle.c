@@ -510,6 +510,64 @@ void g3o_qtet_frame(const int32_t *m, int64_t n, int32_t n_q, uint64_t *H, uint6
     stats[1] += skipped;
 }
 
+/* ------------------------------------------------------------------------- */
+/* MSD: the mean square displacement over all time origins, Eq. 5
+ * and Algorithm 10: "Starting from unwrapped" positions, loop
+ * over the particles, over the time interval dt = 0 .. and over the origins t = 1 .. Nframe-dt,
+ * "Compute MSD of particle between t and t+dt", "Accumulate MSD array".
+ * Readings (M1-M3; the paper states none of these):
+ *  M1 positions are snapped to the box/2^20 grid WITHOUT wrapping, m = llrint(x * 2^20 / box),
+ *     so every squared displacement is an integer and the sums are exact; |m| < 2^30 is required
+ *     (returns the number of coordinates outside, and no result, otherwise);
+ *  M2 S[dt] = sum_i sum_{t=0}^{F-dt-1} |m_i(t+dt) - m_i(t)|^2 as a 128-bit integer, returned as
+ *     (lo, hi) 64-bit words; lags dt = 0 .. max_lag, max_lag <= F - 1;
+ *  M3 msd[dt] = (hi 2^64 + lo) g^2 / (N (F - dt)) in fp64, g = box / 2^20, evaluated as
+ *     s = (double)hi * 2^64 + (double)lo; num = s * (g * g); den = (double)N * (double)(F - dt);
+ *     msd = num / den.
+ * pos [F][n][3] fp64; sums [max_lag+1][2]; msd [max_lag+1].                                  */
+int64_t g3o_msd(const double *pos, int64_t n_frames, int64_t n, double box, int64_t max_lag,
+                uint64_t *sums, double *msd)
+{
+    double inv_g = 1048576.0 / box;
+    int64_t total = n_frames * n * 3, bad = 0;
+    int64_t *m = (int64_t *)malloc(sizeof(int64_t) * (size_t)total);
+    for (int64_t q = 0; q < total; ++q) {
+        m[q] = (int64_t)llrint(pos[q] * inv_g);
+        if (m[q] >= ((int64_t)1 << 30) || m[q] <= -((int64_t)1 << 30)) bad += 1;
+    }
+    if (bad) { free(m); return bad; }
+    unsigned __int128 *S = (unsigned __int128 *)calloc((size_t)(max_lag + 1), sizeof(unsigned __int128));
+#pragma omp parallel
+    {
+        unsigned __int128 *loc = (unsigned __int128 *)calloc((size_t)(max_lag + 1), sizeof(unsigned __int128));
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i)                       /* Loop 1 over the particles      */
+            for (int64_t dt = 0; dt <= max_lag; ++dt)         /* Loop 2 over the time interval  */
+                for (int64_t t = 0; t < n_frames - dt; ++t) { /* Loop 3 over the origins        */
+                    const int64_t *a = m + ((t * n) + i) * 3, *b = m + (((t + dt) * n) + i) * 3;
+                    int64_t dx = b[0] - a[0], dy = b[1] - a[1], dz = b[2] - a[2];
+                    loc[dt] += (unsigned __int128)(uint64_t)(dx * dx + dy * dy + dz * dz);
+                }
+#pragma omp critical
+        for (int64_t dt = 0; dt <= max_lag; ++dt) S[dt] += loc[dt];
+        free(loc);
+    }
+    double g = box / 1048576.0;
+    double gg = g * g;
+    for (int64_t dt = 0; dt <= max_lag; ++dt) {
+        uint64_t lo = (uint64_t)S[dt], hi = (uint64_t)(S[dt] >> 64);
+        sums[2 * dt + 0] = lo;
+        sums[2 * dt + 1] = hi;
+        double s = (double)hi * 18446744073709551616.0 + (double)lo;
+        double num = s * gg;
+        double den = (double)n * (double)(n_frames - dt);
+        msd[dt] = num / den;
+    }
+    free(S);
+    free(m);
+    return 0;
+}
+
 int32_t g3o_num_threads(void)
 {
 #ifdef _OPENMP

@@ -47,6 +47,8 @@ def _load() -> C.CDLL:
         _lib.g3o_g2_normalise.restype = None
         _lib.g3o_qtet_frame.argtypes = [i32p, C.c_int64, C.c_int32, u64p, u64p, f64p]
         _lib.g3o_qtet_frame.restype = None
+        _lib.g3o_msd.argtypes = [f64p, C.c_int64, C.c_int64, C.c_double, C.c_int64, u64p, f64p]
+        _lib.g3o_msd.restype = C.c_int64
         _lib.g3o_num_threads.restype = C.c_int32
         for fn in (_lib.g3o_thresholds, _lib.g3o_quantise, _lib.g3o_accumulate, _lib.g3o_volumes,
                    _lib.g3o_normalise):
@@ -162,6 +164,22 @@ def qtet_frame(m: np.ndarray, n_q: int, H: Optional[np.ndarray] = None,
     qp = _p(q_out, C.c_double) if q_out is not None else None
     _load().g3o_qtet_frame(_p(m, C.c_int32), m.shape[0], n_q, _p(H, C.c_uint64), _p(stats, C.c_uint64), qp)
     return H, stats
+
+
+def msd(pos: np.ndarray, box: float, max_lag: Optional[int] = None):
+    """(sums uint64 [max_lag+1, 2] = (lo, hi) of the exact 128-bit sums of squared grid
+    displacements, msd fp64 [max_lag+1]) of an UNWRAPPED trajectory pos [F, n, 3] (g3o_msd)."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    F, n, three = pos.shape
+    assert three == 3
+    L = F - 1 if max_lag is None else int(max_lag)
+    assert 0 <= L <= F - 1
+    sums = np.zeros((L + 1, 2), dtype=np.uint64)
+    out = np.zeros(L + 1, dtype=np.float64)
+    bad = _load().g3o_msd(_p(pos, C.c_double), F, n, box, L, _p(sums, C.c_uint64), _p(out, C.c_double))
+    if bad:
+        raise ValueError(f"{bad} coordinates outside +-2^30 grid units")
+    return sums, out
 
 
 class Oracle:

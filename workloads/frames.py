@@ -157,3 +157,13 @@ def uniform_frame(n: int, seed: int) -> np.ndarray:
     """int32 [n, 3] uniform random grid coordinates (ideal gas) for ad-hoc test sizes."""
     rng = np.random.default_rng(seed)
     return rng.integers(0, GRID, size=(n, 3), dtype=np.int64).astype(np.int32)
+
+
+def unwrapped_walk(n: int, n_frames: int, seed: int, step_sigma: float = 1000.0) -> np.ndarray:
+    """int64 [F, n, 3] UNWRAPPED grid coordinates of a Gaussian random walk (for the MSD path,
+    PAPER.md:642 "Starting from unwrapped"): uniform start in the box, then integer steps
+    rint(N(0, step_sigma)) per coordinate and frame, never wrapped.  No method arithmetic."""
+    rng = np.random.default_rng(seed)
+    start = rng.integers(0, GRID, size=(1, n, 3), dtype=np.int64)
+    steps = np.rint(rng.normal(scale=step_sigma, size=(n_frames - 1, n, 3))).astype(np.int64)
+    return np.concatenate([start, start + np.cumsum(steps, axis=0)], axis=0)
