@@ -194,6 +194,20 @@ G3_API int g3_normalize(g3_plan *p, const uint64_t *d_counts, uint64_t frames, d
  * length) to host memory.                                                           */
 G3_API int g3_bin_volumes(const g3_plan *p, double *h_volumes);
 
+/* Mean square displacement over all time origins (Eq. 5; Algorithms 10-11,
+ * PAPER.md:642-702) of an UNWRAPPED trajectory; no plan is needed.  DESIGN.md readings M1-M3:
+ * positions are snapped to the box/2^20 grid without wrapping (|x| < 1024 box lengths), so
+ *   S[dt] = sum_i sum_{t=0}^{F-dt-1} |m_i(t+dt) - m_i(t)|^2,  dt = 0 .. max_lag <= F - 1,
+ * is an exact 128-bit integer, and msd[dt] = S[dt] (box/2^20)^2 / (n (F - dt)).
+ *   d_pos    device, fp64 [n_frames][n][3], frame f at d_pos + f * frame_stride (>= 3 n doubles)
+ *   d_sums   device, uint64 [max_lag + 1][2] = (low, high) words of S; may be NULL
+ *   d_msd    device, fp64 [max_lag + 1], in the length unit of `box` squared; may be NULL
+ * Stream-ordered work, then SYNCHRONISES `stream` (scratch comes from the stream's memory pool).
+ * Errors: G3_EINVAL (arguments, or a coordinate outside the grid range: outputs are then
+ * meaningless), G3_ENOMEM, G3_ECUDA.                                                       */
+G3_API int g3_msd(const double *d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
+                  int64_t max_lag, uint64_t *d_sums, double *d_msd, void *stream);
+
 /* Measure, on the current device, one of the two ceilings the triplet kernel's roofline is
  * quoted against: which = 0, shared-memory atomic increments per
  * second over the whole GPU for pseudo-random slots of a `slots`-word tile (bank conflicts

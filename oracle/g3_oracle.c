@@ -546,7 +546,7 @@ int64_t g3o_msd(const double *pos, int64_t n_frames, int64_t n, double box, int6
                 for (int64_t t = 0; t < n_frames - dt; ++t) { /* Loop 3 over the origins        */
                     const int64_t *a = m + ((t * n) + i) * 3, *b = m + (((t + dt) * n) + i) * 3;
                     int64_t dx = b[0] - a[0], dy = b[1] - a[1], dz = b[2] - a[2];
-                    loc[dt] += (unsigned __int128)(uint64_t)(dx * dx + dy * dy + dz * dz);
+                    loc[dt] += (unsigned __int128)((uint64_t)(dx * dx) + (uint64_t)(dy * dy) + (uint64_t)(dz * dz));
                 }
 #pragma omp critical
         for (int64_t dt = 0; dt <= max_lag; ++dt) S[dt] += loc[dt];

@@ -24,7 +24,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_msd", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -65,6 +65,7 @@ def load() -> C.CDLL:
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
     lib.g3_microbench.argtypes = [i32, i64, i64, C.POINTER(f64), vp]
+    lib.g3_msd.argtypes = [vp, i64, i64, i64, f64, i64, vp, vp, vp]
     lib.g3_plan_reset.argtypes = [vp, vp]
     lib.g3_plan_destroy.argtypes = [vp]
     lib.g3_plan_destroy.restype = None
@@ -100,6 +101,22 @@ def microbench(which: int, slots: int = 50776, iters: int = 1 << 14, stream=None
     _check(load().g3_microbench(int(which), int(slots), int(iters), C.byref(rate), _stream_ptr(stream)),
            "g3_microbench")
     return float(rate.value)
+
+
+def msd(d_pos, box: float, max_lag: Optional[int] = None, stream=None):
+    """g3_msd of an unwrapped fp64 cuda trajectory [F, n, 3]: (sums int64-viewed-as-uint64
+    [max_lag+1, 2] = (low, high) words, msd fp64 [max_lag+1]) device tensors."""
+    import torch
+    if d_pos.dtype != torch.float64 or d_pos.device.type != "cuda" or not d_pos.is_contiguous() or \
+            d_pos.dim() != 3 or d_pos.shape[2] != 3:
+        raise ValueError("positions must be a contiguous float64 cuda tensor [F, n, 3]")
+    F, n = int(d_pos.shape[0]), int(d_pos.shape[1])
+    L = F - 1 if max_lag is None else int(max_lag)
+    sums = torch.empty((L + 1, 2), dtype=torch.int64, device="cuda")
+    out = torch.empty(L + 1, dtype=torch.float64, device="cuda")
+    _check(load().g3_msd(d_pos.data_ptr(), F, n, 3 * n, float(box), L, sums.data_ptr(), out.data_ptr(),
+                         _stream_ptr(stream)), "g3_msd")
+    return sums, out
 
 
 class Plan:

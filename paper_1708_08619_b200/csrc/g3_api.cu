@@ -18,6 +18,7 @@
 #include "g3_cells.cuh"
 #include "g3_generic.cuh"
 #include "g3_microbench.cuh"
+#include "g3_msd.cuh"
 #include "g3_plan.h"
 #include "g3_qtet.cuh"
 #include "g3_tiled.cuh"
@@ -597,6 +598,55 @@ int g3_microbench(int32_t which, int64_t slots, int64_t iters, double* h_rate, v
     // thread-level operations per second over the whole GPU (loop overhead not counted)
     *h_rate = (double)grid * kMbThreads * (double)it / ((double)ms * 1e-3);
     return G3_OK;
+}
+
+int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
+           int64_t max_lag, uint64_t* d_sums, double* d_msd, void* stream) {
+    if (!d_pos || n_frames < 1 || n < 1 || n > (int64_t(1) << 30) || n_frames > (int64_t(1) << 24) ||
+        frame_stride < 3 * n || !(box > 0.0) || !std::isfinite(box) || max_lag < 0 || max_lag > n_frames - 1)
+        return G3_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, cc_major = 0, smem_optin = 0, sm_count = 0;    // (cudaGetDeviceProperties takes ms)
+    G3_CUDA(cudaGetDevice(&dev));
+    G3_CUDA(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    G3_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    G3_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    if (cc_major < 10) return G3_ECUDA;
+    const int32_t n_blocks = (int32_t)((n + kMsdAtoms - 1) / kMsdAtoms);
+    const size_t traj_smem = (size_t)n_frames * kMsdAtoms * 3 * sizeof(int32_t);
+    const bool smem_path = traj_smem <= (size_t)smem_optin;
+    MsdParams mp;
+    mp.pos = d_pos; mp.stride = frame_stride; mp.n = (int32_t)n; mp.n_frames = (int32_t)n_frames;
+    mp.max_lag = (int32_t)max_lag; mp.inv_g = 1048576.0 / box; mp.snapped = nullptr;
+    void* ws = nullptr;                   // partials | bad counter | snapped copy (global path)
+    const size_t part_bytes = sizeof(ulonglong2) * (size_t)n_blocks * (size_t)(max_lag + 1);
+    const size_t snap_bytes = smem_path ? 0 : sizeof(int32_t) * 3 * (size_t)n * (size_t)n_frames;
+    G3_CUDA(cudaMallocAsync(&ws, part_bytes + 16 + snap_bytes, st));
+    mp.partial = reinterpret_cast<ulonglong2*>(ws);
+    mp.bad = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws) + part_bytes);
+    int rc = G3_OK;
+    auto fail = [&](int code) { cudaFreeAsync(ws, st); cudaGetLastError(); return code; };
+    if (cudaMemsetAsync(mp.bad, 0, 16, st) != cudaSuccess) return fail(G3_ECUDA);
+    if (smem_path) {
+        if (cudaFuncSetAttribute(msd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)traj_smem) != cudaSuccess) return fail(G3_ECUDA);
+        msd_kernel<true><<<n_blocks, kMsdWarps * 32, traj_smem, st>>>(mp);
+    } else {
+        mp.snapped = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + part_bytes + 16);
+        msd_snap_kernel<<<sm_count * 8, 256, 0, st>>>(mp);
+        msd_kernel<false><<<n_blocks, kMsdWarps * 32, 0, st>>>(mp);
+    }
+    const double g = box / 1048576.0;
+    msd_reduce_kernel<<<(unsigned)((max_lag + 128) / 128), 128, 0, st>>>(
+        mp.partial, n_blocks, (int32_t)max_lag, (int32_t)n, (int32_t)n_frames, g * g,
+        reinterpret_cast<unsigned long long*>(d_sums), d_msd);
+    if (cudaGetLastError() != cudaSuccess) return fail(G3_ECUDA);
+    unsigned long long bad = 0;
+    if (cudaMemcpyAsync(&bad, mp.bad, sizeof(bad), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) return fail(G3_ECUDA);
+    cudaFreeAsync(ws, st);
+    if (bad) rc = G3_EINVAL;              // coordinates outside +-2^30 grid units: results invalid
+    return rc;
 }
 
 int g3_bin_volumes(const g3_plan* p, double* h_volumes) {
