@@ -336,6 +336,26 @@ def run_ours(args):
                     "atoms_per_s_extra": qs[0] / (extra * 1e-3), "bins": 200}
     except Exception as e:  # the g3 numbers above stay valid
         qtet = {"error": str(e)}
+    # MSD over all time origins at the same shape (unwrapped random walk,
+    # N = 32768, F frames, every lag), device-resident; CUDA events around the g3_msd calls
+    msd = None
+    try:
+        from workloads import unwrapped_walk
+        d_walk = torch.from_numpy(grid_to_pos(unwrapped_walk(w.n, F, seed=w.seed), w.box)).cuda()
+        g3.msd(d_walk, w.box)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(3):
+            g3.msd(d_walk, w.box)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_msd = e0.elapsed_time(e1) / 3
+        disp = w.n * F * (F + 1) // 2
+        msd = {"ms": ms_msd, "displacements_per_s": disp / (ms_msd * 1e-3), "frames": F, "lags": F,
+               "hbm_gbs_achieved": F * w.n * 24 / (ms_msd * 1e-3) / 1e9}
+        del d_walk
+    except Exception as e:  # the g3 numbers above stay valid
+        msd = {"error": str(e)}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu, _, _, _ = cpu_baseline_leg(w, args.cpu_budget)
@@ -360,6 +380,7 @@ def run_ours(args):
         "gpu_launches_per_step": launches,
         "roofline": roofline,
         "qtet": qtet,
+        "msd": msd,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
