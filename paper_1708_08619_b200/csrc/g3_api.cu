@@ -201,8 +201,13 @@ int flush(g3_plan* p, cudaStream_t st) {
         if (p->d_qtet_redo) {
             G3_CUDA(cudaMemsetAsync(p->d_qtet_redo, 0, sizeof(int32_t), st));
             const long long items = (long long)nc3 * F;
-            qtet_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->sm_count * 8), kQtCellWarps * 32,
-                               qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins), st>>>(fb, qp);
+            // persistent: exactly the CTAs that are resident together (a larger grid would run a second wave)
+            const size_t cell_smem = qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins);
+            int per_sm = 0;
+            G3_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qtet_cell_kernel, kQtCellWarps * 32, cell_smem));
+            per_sm = std::max(per_sm, 1);
+            qtet_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->sm_count * per_sm), kQtCellWarps * 32,
+                               cell_smem, st>>>(fb, qp);
             qp.use_redo = 1;                               // the few atoms the fast path could not decide
             qtet_redo_kernel<kQtetWarps><<<(unsigned)p->sm_count * 2, kQtetWarps * 32, hist_smem, st>>>(fb, qp);
             p->launches += 2;
