@@ -112,8 +112,9 @@ int configure(g3_plan* p) {
     p->max_nb = (int32_t)cap;
 
     if (p->batch_auto) {
-        // small frames are launch-bound: stage enough frames for ~2^19 centres per launch sequence
-        const int64_t want = ((int64_t(1) << 19) + p->n - 1) / p->n;
+        // every triplet launch zeroes and flushes a whole histogram tile per CTA (~75 us at 64^3
+        // bins): stage enough frames for ~2^21 centres per launch sequence
+        const int64_t want = ((int64_t(1) << 21) + p->n - 1) / p->n;
         p->batch_frames = (int32_t)std::min<int64_t>(std::max<int64_t>(want, 16), 256);
     }
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled
@@ -676,7 +677,7 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     }
     if (p->tiled) {
         G3_CUDA(cudaMemsetAsync(p->tiled->d_scratch, 0,
-                                sizeof(unsigned long long) * (p->tiled->tile_bins + p->bins.n_r) * p->tiled->grid, st));
+                                sizeof(unsigned long long) * p->tiled->tile_bins * p->tiled->grid, st));
         p->tiled->dirty = false;
     }
     p->pending = 0;

@@ -32,7 +32,8 @@ struct TiledState {
     uint32_t* d_slot_map = nullptr;            // [tile_bins] packed (a, b, c); 0xFFFFFFFF = unused
     unsigned long long* d_scratch = nullptr;   // [grid][tile_bins] per-CTA partial tiles
     // neighbour lists of one batch
-    float4* d_nbv = nullptr;                   // [batch][n][max_nb] (dx, dy, dz, shell)
+    float4* d_nbv = nullptr;                   // [batch][n][max_nb] (dx, dy, dz, addend(shell))
+    uint32_t* d_nbj = nullptr;                 // [batch][n][max_nb] row offset of the shell
     int32_t* d_nbcount = nullptr;              // [batch][n]
     unsigned int* d_work = nullptr;            // work-queue counter
     int4* d_cell_origin = nullptr;             // [ncell3] cell centres on the grid
@@ -121,15 +122,15 @@ inline void build_layout(const g3_plan* p, TiledState& ts) {
 // ---------------------------------------------------------------------------------------------
 // host side
 inline int32_t tiled_stage_cap(const g3_plan* p) {
-    if (p->ncell == 1) return (int32_t)((p->n + 31) / 32 * 32);
+    if (p->ncell == 1) return (int32_t)((p->n + 63) / 64 * 64);
     // twice the mean occupancy of 27 cells; more crowded neighbourhoods are read from global
     const double per27 = 27.0 * (double)p->n / ((double)p->ncell * p->ncell * p->ncell);
     const int64_t cap = (int64_t)(2.0 * per27) + 96;
-    return (int32_t)((cap + 31) / 32 * 32);
+    return (int32_t)((cap + 63) / 64 * 64);
 }
 
 inline int tiled_warps(const g3_plan* p, int64_t tile_bins) {
-    int w = p->tri_warps_opt ? p->tri_warps_opt : 20;   // 20 warps x 96 registers: no spills (measured best)
+    int w = p->tri_warps_opt ? p->tri_warps_opt : 16;   // 16 warps x 128 registers: no spills (measured best)
     while (w > 8 && tri_smem_bytes(tile_bins, w, p->bins.n_r) > (size_t)p->smem_optin) w -= 4;
     return w;
 }
@@ -150,7 +151,7 @@ inline bool tiled_plan_slabs(const g3_plan* p, TiledState& ts) {
         ts.slab_bins_max = ts.tile_bins;
         return true;
     }
-    const int warps = p->tri_warps_opt ? p->tri_warps_opt : 20;
+    const int warps = p->tri_warps_opt ? p->tri_warps_opt : 16;
     return build_slabs(ts, p->bins.n_r, tiled_cap_slots(p, warps)) && ts.n_slabs <= 64;
 }
 
@@ -170,7 +171,7 @@ inline void tiled_free(g3_plan* p) {
     TiledState* ts = p->tiled;
     if (!ts) return;
     cudaFree(ts->d_addend); cudaFree(ts->d_jconst); cudaFree(ts->d_slot_map); cudaFree(ts->d_scratch);
-    cudaFree(ts->d_nbv); cudaFree(ts->d_nbcount); cudaFree(ts->d_work); cudaFree(ts->d_cell_origin);
+    cudaFree(ts->d_nbv); cudaFree(ts->d_nbj); cudaFree(ts->d_nbcount); cudaFree(ts->d_work); cudaFree(ts->d_cell_origin);
     cudaFree(ts->d_slab_shell); cudaFree(ts->d_slabpos);
     delete ts;
     p->tiled = nullptr;
@@ -222,7 +223,7 @@ inline int tiled_configure(g3_plan* p) {
     if (ts->max_batch_frames < 1) return G3_EINVAL;
     if (p->batch_frames > ts->max_batch_frames) p->batch_frames = (int32_t)ts->max_batch_frames;
     // neighbour lists of one batch: keep them below ~16 GiB
-    const size_t frame_bytes = (size_t)p->n * p->max_nb * sizeof(float4);
+    const size_t frame_bytes = (size_t)p->n * p->max_nb * (sizeof(float4) + sizeof(uint32_t));
     const int64_t mem_frames = std::max<int64_t>(1, (int64_t)((size_t(16) << 30) / frame_bytes));
     if (p->batch_frames > mem_frames) p->batch_frames = (int32_t)mem_frames;
 
@@ -253,8 +254,10 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMalloc(&ts->d_addend, sizeof(float) * n_r));
     G3T_CUDA(cudaMalloc(&ts->d_jconst, sizeof(int32_t) * n_r));
     G3T_CUDA(cudaMalloc(&ts->d_slot_map, sizeof(uint32_t) * ts->tile_bins));
-    G3T_CUDA(cudaMalloc(&ts->d_scratch, sizeof(unsigned long long) * (ts->tile_bins + n_r) * ts->grid));
+    G3T_CUDA(cudaMalloc(&ts->d_scratch, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
     G3T_CUDA(cudaMalloc(&ts->d_nbv, sizeof(float4) * (per_frame_entries * B + 64)));   // +64: prefetch overrun
+    G3T_CUDA(cudaMalloc(&ts->d_nbj, sizeof(uint32_t) * (per_frame_entries * B + 64)));
+    G3T_CUDA(cudaMemset(ts->d_nbj, 0, sizeof(uint32_t) * (per_frame_entries * B + 64)));
     G3T_CUDA(cudaMalloc(&ts->d_nbcount, sizeof(int32_t) * (size_t)p->n * B));
     G3T_CUDA(cudaMalloc(&ts->d_work, sizeof(unsigned int)));
     if (ts->n_slabs > 1) {
@@ -272,14 +275,15 @@ inline int tiled_configure(g3_plan* p) {
                     origin[((size_t)cx * nc + cy) * nc + cz] =
                         make_int4((int32_t)(((int64_t)(2 * cx + 1) << (kGridBits - 1)) / nc),
                                   (int32_t)(((int64_t)(2 * cy + 1) << (kGridBits - 1)) / nc),
-                                  (int32_t)(((int64_t)(2 * cz + 1) << (kGridBits - 1)) / nc), 0);
+                                  (int32_t)(((int64_t)(2 * cz + 1) << (kGridBits - 1)) / nc),
+                                  cx | (cy << 8) | (cz << 16));
         G3T_CUDA(cudaMalloc(&ts->d_cell_origin, sizeof(int4) * origin.size()));
         G3T_CUDA(cudaMemcpy(ts->d_cell_origin, origin.data(), sizeof(int4) * origin.size(), cudaMemcpyHostToDevice));
     }
     G3T_CUDA(cudaMemcpy(ts->d_addend, addend.data(), sizeof(float) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_jconst, jconst.data(), sizeof(int32_t) * n_r, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemcpy(ts->d_slot_map, slot_map.data(), sizeof(uint32_t) * ts->tile_bins, cudaMemcpyHostToDevice));
-    G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * (ts->tile_bins + n_r) * ts->grid));
+    G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
     G3T_CUDA(cudaMemset(ts->d_nbv, 0, sizeof(float4) * (per_frame_entries * B + 64)));
     G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
     G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
@@ -295,9 +299,9 @@ inline int tiled_configure(g3_plan* p) {
 inline int tiled_merge(g3_plan* p, cudaStream_t st) {
     TiledState* ts = p->tiled;
     if (!ts || !ts->dirty) return G3_OK;
-    merge_kernel<<<(unsigned)((ts->tile_bins + p->bins.n_r + 255) / 256), 256, 0, st>>>(
+    merge_kernel<<<(unsigned)((ts->tile_bins + 255) / 256), 256, 0, st>>>(
         ts->d_scratch, ts->d_slot_map, (int32_t)ts->tile_bins, ts->grid, p->bins.n_r, p->bins.n_t,
-        p->d_counts, p->d_counts2, p->d_stats);
+        p->d_counts, p->d_stats);
     p->launches += 1;
     ts->dirty = false;
     G3T_CUDA(cudaGetLastError());
@@ -319,7 +323,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     np.inv_w_hi = (float)((1.0 / w) * (1.0 + eps));
     np.T_r = bs.T_r;
     np.cell_origin = ts->d_cell_origin;
-    np.nbv = ts->d_nbv; np.nbcount = ts->d_nbcount; np.stats = p->d_stats;
+    np.nbv = ts->d_nbv; np.nbj = ts->d_nbj; np.addend = ts->d_addend; np.jconst = ts->d_jconst; np.nbcount = ts->d_nbcount; np.stats = p->d_stats; np.counts2 = p->d_counts2;
     np.n_slabs = ts->n_slabs; np.slab_shell = ts->d_slab_shell; np.slabpos = ts->d_slabpos;
     G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -348,10 +352,9 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     tp.cta_item_cap = ts->cta_item_cap;
     tp.inv_lo = (float)((1.0 / wt) * (1.0 - eps));
     tp.inv_hi = (float)((1.0 / wt) * (1.0 + eps));
-    tp.T_t = bs.T_t; tp.nbv = ts->d_nbv; tp.nbcount = ts->d_nbcount;
-    tp.addend = ts->d_addend; tp.jconst = ts->d_jconst;
+    tp.T_t = bs.T_t; tp.nbv = ts->d_nbv; tp.nbj = ts->d_nbj; tp.nbcount = ts->d_nbcount;
     tp.work = ts->d_work;
-    tp.scratch_stride = ts->tile_bins + bs.n_r;
+    tp.scratch_stride = ts->tile_bins;
     tp.n_slabs = ts->n_slabs; tp.slabpos = ts->d_slabpos;
     for (int32_t s = 0; s < ts->n_slabs; ++s) {
         const int32_t b0 = ts->slab_shell[s], b1 = ts->slab_shell[s + 1];
@@ -359,7 +362,6 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         tp.slot_base = ts->BASE[b0];
         tp.tile_bins = ts->n_slabs > 1 ? ts->BASE[b1] - ts->BASE[b0] + 2 : (int32_t)ts->tile_bins;
         tp.scratch = ts->d_scratch + tp.slot_base;
-        tp.g2_out = ts->tile_bins - tp.slot_base;
         if (s > 0) G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
         switch (ts->tri_warps) {
             case 24: tiled_launch_triplet<24>(ts, tp, st); break;

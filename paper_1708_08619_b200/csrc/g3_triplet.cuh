@@ -1,18 +1,21 @@
 // g3_triplet.cuh -- steps a4 + a5: the triplet kernel (Algorithm 7 CUDA_g3)
 // and the merge of its per-CTA partial histograms.
 //
-// tiled_triplet_kernel: persistent, one CTA per SM.  A warp per centre; lane = neighbour j
-// (32 at a time), the partner k is broadcast from a 32-entry shared-memory window; every
-// UNORDERED pair j < k is visited once (the lists are sorted by shell, so a_j <= a_k) and
-// counted with one shared-memory atomic into a privatised histogram tile that holds only the
+// tiled_triplet_kernel: persistent, one CTA per SM, a warp per centre.  The centre's neighbour
+// list (sorted by shell, so a_j <= a_k for j < k; written by neighbour_kernel already in window
+// form) is staged in a per-warp shared-memory window; every UNORDERED pair j < k is visited once
+// and counted with one shared-memory atomic into a privatised histogram tile that holds only the
 // bins the triangle inequality allows:
 //     slot(a, b, c) = 1 + BASE(b) + P(a) + c - g(b) + h(a)          (a <= b)
-// (DESIGN.md section 4.3).  Slot 0 is a guard: lanes without a pair in an iteration add to it,
-// so every shared atomic is issued by a full, converged warp (measured on B200: a full-warp
-// ATOMS.POPC.INC retires in 2.0-2.7 SM cycles, a partially predicated one in 4.1 with ~90
-// cycles of latency).  The list of the NEXT centre is loaded into registers while the current
-// one is processed.  When the kernel ends each CTA adds its tile to its own uint64 partial
-// tile in global memory; merge_kernel mirrors the partial tiles into the [a][b][c] histogram.
+// (DESIGN.md section 5.3).  The k side of a pair comes from the window as (x, y, z, addend(b)),
+// the j side is held in registers as (x, y, z, row offset(a)): four j entries per lane
+// (g, g + 8, g + 16, g + 24 of a 32-block, g = lane & 7), so that one quarter-warp broadcast load
+// of a k entry serves four pairs.  Slot 0 is a guard: lanes without a pair in an iteration add
+// to it, so every shared atomic is issued by a full, converged warp (measured on B200: a
+// full-warp ATOMS.POPC.INC retires in 2.3-2.8 SM cycles whatever the bank conflicts, a partially
+// predicated one in 4.1).  The list of the NEXT centre is loaded into registers while the current
+// one is processed.  When the kernel ends each CTA adds its tile to its own uint64 partial tile
+// in global memory; merge_kernel mirrors the partial tiles into the [a][b][c] histogram.
 //
 // Exactness.  Differences of neighbour vectors are exact in fp32 (integers below 2^21).  The
 // squared distance, its square root and the bin index are computed in fp32 with a relative
@@ -27,6 +30,8 @@
 namespace g3 {
 
 constexpr int kItemCentres = 8;                // centres per work-queue fetch
+constexpr int kWinEntries = 64;                // entries of a warp's window
+constexpr int kWinBytes = kWinEntries * 20;    // (x, y, z, addend) + row offset per entry
 
 struct TriParams {
     long long total_centres;              // frames * n
@@ -35,16 +40,14 @@ struct TriParams {
     uint32_t cta_item_cap;                // items one CTA may take (u32 tile slots cannot overflow)
     float inv_lo, inv_hi;                 // (1/wt)(1 -+ 2^-20), wt = t-bin width in grid units
     const unsigned long long* T_t;
-    const float4* nbv;                    // [centres][max_nb] (dx, dy, dz, shell)
+    const float4* nbv;                    // [centres][max_nb] (dx, dy, dz, addend(shell))
+    const uint32_t* nbj;                  // [centres][max_nb] 4 * (P(shell) + h(shell))
     const int32_t* nbcount;
-    const float* addend;                  // [n_r]  kMagic + BASE(b) - g(b) + 1
-    const int32_t* jconst;                // [n_r]  4 * (P(a) + h(a))
     unsigned int* work;
     unsigned long long* scratch;          // [grid][scratch_stride], already offset by slot_base
     // slab passes (kSlab kernels): this launch counts only pairs whose outer member k lies in
     // the shell range of slab `slab`; its tile holds the slots slot_base+1 .. slot_base+tile_bins-2
-    long long scratch_stride;             // slots of one CTA's partial tile: whole layout + n_r (g2)
-    long long g2_out;                     // offset of the g2 slots from `scratch` (pre-offset pointer)
+    long long scratch_stride;             // slots of one CTA's partial tile: the whole layout
     int32_t slot_base;                    // BASE(first shell of the slab)
     int32_t n_slabs, slab;
     const int32_t* slabpos;               // [centres][n_slabs + 1] list position where each slab starts
@@ -81,7 +84,7 @@ __device__ __noinline__ void fix_pair(float4 kv, float jx, float jy, float jz, u
     }
 }
 
-// The j side of a pair: vector and the tile byte offset of its shell row.
+// The j side of a pair: vector and the tile byte address of its shell row (window base folded in).
 struct JSide {
     float x, y, z;
     uint32_t J;
@@ -120,45 +123,57 @@ __device__ __forceinline__ void four_pairs(const TriParams& tp, uint32_t guard,
     }
 }
 
+// The four j entries a lane holds of the 32-block at `win`: g, g + 8, g + 16, g + 24 (g = lane & 7).
+struct JQuad {
+    JSide j[4];
+};
+
+__device__ __forceinline__ JQuad load_jquad(const float4* __restrict__ win, const uint32_t* __restrict__ winJ, int lane) {
+    JQuad q;
+    const int g = lane & 7;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) q.j[m] = load_jside(win, winJ, g + 8 * m);
+    return q;
+}
+
 // All unordered pairs inside one 32-block of a neighbour list whose entries 0..kt-1 are valid
-// (16 < kt <= 32) and staged in `win` (vectors + addends) and `winJ` (row offsets).
-// Recursive halving: at level H (16, 8, 4, 2, 1) the block splits into aligned sub-blocks of 2H
-// entries and every pair whose members first differ in bit H is visited, j from the lower half
-// (so j < k and a_j <= a_k), k from the upper half.  Each level is an H x H rectangle per
-// sub-block; levels 16, 8 and 4 are register-tiled 2 j x n k per lane, so one broadcast load of
-// a k entry serves two pairs (the shared-memory data pipe, not the issue slots, binds this
-// kernel: DESIGN.md section 5).  A full block takes 16 pair slots per lane for its 496 pairs
-// (97 % of the lane slots used); the lane-vs-broadcast triangle it replaces took 31 (50 %).
+// (16 < kt <= 32) and staged in `win` (vectors + addends) and `winJ` (row offsets); `q` = the
+// block's j entries this lane holds.  Recursive halving: at level H (16, 8, 4, 2, 1) the block
+// splits into aligned sub-blocks of 2H entries and every pair whose members first differ in bit H
+// is visited, j from the lower half (so j < k and a_j <= a_k), k from the upper half.  Each level
+// is an H x H rectangle per sub-block.  Levels 16 and 8 take their j side from `q`; their k side
+// is one address per quarter-warp.  A full block takes 16 pair slots per lane for its 496 pairs
+// (97 % of the lane slots used); a lane-vs-broadcast triangle would take 31 (50 %).
 template <bool kFull>
 __device__ __forceinline__ void triangle32(const TriParams& tp, const float4* __restrict__ win,
                                            const uint32_t* __restrict__ winJ, uint32_t guard,
-                                           int lane, int32_t kt, const JSide& own) {
-    {   // H = 16: j = {g, g + 8}, k = 16 + kg + 4 it, it = 0..3
-        const int g = lane & 7, kidx = 16 + (lane >> 3);
-        const JSide ja = load_jside(win, winJ, g), jb = load_jside(win, winJ, g + 8);
+                                           int lane, int32_t kt, const JQuad& q) {
+    const int kq = lane >> 3;
+    {   // H = 16: j = {g, g + 8}, k = 16 + kq + 4 it, it = 0..3
+        const int kidx = 16 + kq;
         {
             const float4 k0 = win[kidx], k1 = win[kidx + 4];
-            four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
-                               kidx < kt, kidx + 4 < kt, kidx < kt, kidx + 4 < kt);
+            four_pairs<!kFull>(tp, guard, k0, k0, k1, k1, q.j[0], q.j[1], q.j[0], q.j[1],
+                               kidx < kt, kidx < kt, kidx + 4 < kt, kidx + 4 < kt);
         }
         if (kFull || kt > 24) {
             const float4 k0 = win[kidx + 8], k1 = win[kidx + 12];
-            four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
-                               kidx + 8 < kt, kidx + 12 < kt, kidx + 8 < kt, kidx + 12 < kt);
+            four_pairs<!kFull>(tp, guard, k0, k0, k1, k1, q.j[0], q.j[1], q.j[0], q.j[1],
+                               kidx + 8 < kt, kidx + 8 < kt, kidx + 12 < kt, kidx + 12 < kt);
         }
     }
-    {   // H = 8, two sub-blocks: j = {b + g, b + g + 4}, k = b + 8 + kg + 4 it, it = 0..1
-        const int b = lane & 16, g = lane & 3, kidx = b + 8 + ((lane >> 2) & 3);
-        const JSide ja = load_jside(win, winJ, b + g), jb = load_jside(win, winJ, b + g + 4);
-        const float4 k0 = win[kidx], k1 = win[kidx + 4];
-        four_pairs<!kFull>(tp, guard, k0, k1, k0, k1, ja, ja, jb, jb,
-                           kidx < kt, kidx + 4 < kt, kidx < kt, kidx + 4 < kt);
+    {   // H = 8: j = g with k = 8 + 2 kq + {0, 1}; j = g + 16 with k = 24 + 2 kq + {0, 1}
+        const int ka = 8 + 2 * kq, kb = 24 + 2 * kq;
+        const float4 k0 = win[ka], k1 = win[ka + 1], k2 = win[kb], k3 = win[kb + 1];
+        four_pairs<!kFull>(tp, guard, k0, k1, k2, k3, q.j[0], q.j[0], q.j[2], q.j[2],
+                           true, true, kb < kt, kb + 1 < kt);
     }
     {   // H = 4 (j = {b + g, b + g + 2}, k = b + 4 + kg), H = 2 and H = 1 (one pair each)
         const int b8 = lane & 24, g = lane & 1, k4 = b8 + 4 + ((lane >> 1) & 3);
         const JSide ja = load_jside(win, winJ, b8 + g), jb = load_jside(win, winJ, b8 + g + 2);
         const int b4 = lane & 28, k2 = b4 + 2 + ((lane >> 1) & 1);
         const JSide jc = load_jside(win, winJ, b4 + g);
+        const JSide own = load_jside(win, winJ, lane);
         const int k1 = lane | 1;
         const float4 kA = win[k4], kB = win[k2], kC = win[k1];
         four_pairs<true>(tp, guard, kA, kA, kB, kC, ja, jb, jc, own,
@@ -188,6 +203,44 @@ __device__ __forceinline__ void triangle16(const TriParams& tp, const float4* __
                      kidx < kt, kidx + 4 < kt, k4 < kt, lane < 24 && kl < kt);
 }
 
+// Rectangle between the 32-block whose j entries are in `q` and the window entries
+// kwin[klo .. kc): k = 4 i + kq per quarter-warp, four pairs (one per held j) per lane.
+__device__ __forceinline__ void rect32(const TriParams& tp, const float4* __restrict__ kwin, uint32_t guard,
+                                       int lane, int32_t klo, int32_t kc, const JQuad& q) {
+    const int kq = lane >> 3;
+    int32_t k0 = klo & ~3;
+    if (k0 < klo) {                                       // slab passes: first group bounded below
+        const int32_t kidx = k0 + kq;
+        const float4 kv = kwin[kidx];
+        const bool p = kidx >= klo && kidx < kc;
+        four_pairs<true>(tp, guard, kv, kv, kv, kv, q.j[0], q.j[1], q.j[2], q.j[3], p, p, p, p);
+        k0 += 4;
+    }
+    for (; k0 + 4 <= kc; k0 += 4) {
+        const float4 kv = kwin[k0 + kq];
+        four_pairs<false>(tp, guard, kv, kv, kv, kv, q.j[0], q.j[1], q.j[2], q.j[3], true, true, true, true);
+    }
+    if (k0 < kc) {
+        const float4 kv = kwin[k0 + kq];
+        const bool p = k0 + kq < kc;
+        four_pairs<true>(tp, guard, kv, kv, kv, kv, q.j[0], q.j[1], q.j[2], q.j[3], p, p, p, p);
+    }
+}
+
+// Rectangle between the 16 entries jwin[0..16) (all valid) and kwin[0..m), 1 <= m <= 16:
+// j = {g, g + 8}, k = 4 i + kq.
+__device__ __forceinline__ void rect16(const TriParams& tp, const float4* __restrict__ jwin,
+                                       const uint32_t* __restrict__ jwinJ, const float4* __restrict__ kwin,
+                                       uint32_t guard, int lane, int32_t m) {
+    const int kq = lane >> 3, g = lane & 7;
+    const JSide ja = load_jside(jwin, jwinJ, g), jb = load_jside(jwin, jwinJ, g + 8);
+    for (int32_t i0 = 0; i0 < m; i0 += 8) {
+        const float4 k0 = kwin[i0 + kq], k1 = kwin[i0 + 4 + kq];
+        const bool p0 = i0 + kq < m, p1 = i0 + 4 + kq < m;
+        four_pairs<true>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, p0, p0, p1, p1);
+    }
+}
+
 // Triangle of a 32-block whose k members are bounded below (slab passes): lane = j, the k
 // members klo <= k < kt are broadcast four at a time.  Runs at most once per centre and slab.
 __device__ __forceinline__ void triangle_from(const TriParams& tp, const float4* __restrict__ win,
@@ -201,35 +254,33 @@ __device__ __forceinline__ void triangle_from(const TriParams& tp, const float4*
     }
 }
 
+// All pairs inside a block of 2 <= kt <= 32 entries at `win`.
+__device__ __forceinline__ void block_pairs(const TriParams& tp, const float4* __restrict__ win,
+                                            const uint32_t* __restrict__ winJ, uint32_t guard,
+                                            int lane, int32_t kt, const JQuad& q) {
+    if (kt == 32) triangle32<true>(tp, win, winJ, guard, lane, kt, q);
+    else if (kt > 16) triangle32<false>(tp, win, winJ, guard, lane, kt, q);
+    else if (kt >= 2) triangle16(tp, win, winJ, guard, lane, kt);
+}
+
 template <int kWarps, bool kSlab>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 tiled_triplet_kernel(TriParams tp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t* tile = reinterpret_cast<uint32_t*>(smem_raw);
-    const size_t tile_bytes = ((size_t)(tp.tile_bins + tp.n_r) * 4 + 15) & ~size_t(15);
-    float4* win_all = reinterpret_cast<float4*>(smem_raw + tile_bytes);       // [warp][2][32]
-    uint32_t* winJ_all = reinterpret_cast<uint32_t*>(win_all + kWarps * 64);  // [warp][32]
-    float* tab_addend = reinterpret_cast<float*>(winJ_all + kWarps * 32);
-    int32_t* tab_j = reinterpret_cast<int32_t*>(tab_addend + tp.n_r);
+    const size_t tile_bytes = ((size_t)tp.tile_bins * 4 + 15) & ~size_t(15);
     __shared__ unsigned int cta_items;
 
-    // the n_r slots after the tile count this CTA's neighbours per shell (g2)
-    for (int32_t i = threadIdx.x; i < tp.tile_bins + tp.n_r; i += blockDim.x) tile[i] = 0;
-    for (int32_t i = threadIdx.x; i < tp.n_r; i += blockDim.x) {
-        tab_addend[i] = tp.addend[i];
-        tab_j[i] = tp.jconst[i];
-    }
+    for (int32_t i = threadIdx.x; i < tp.tile_bins; i += blockDim.x) tile[i] = 0;
     if (threadIdx.x == 0) cta_items = 0;
     __syncthreads();
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float4* winA = win_all + wid * 64;          // the 32-block the j side comes from
-    float4* winB = winA + 32;                   // the later 32-block the k side comes from
-    uint32_t* winJ = winJ_all + wid * 32;       // tile row offsets of winA's entries
+    float4* win = reinterpret_cast<float4*>(smem_raw + tile_bytes + (size_t)wid * kWinBytes);   // [64] k side
+    uint32_t* winJ = reinterpret_cast<uint32_t*>(win + kWinEntries);                             // [64] row addresses
     const uint32_t guard = (uint32_t)__cvta_generic_to_shared(tile);      // slot 0
     // shared-window byte address of slot 0 minus the magic bits (mod 2^32), see file header
     const uint32_t cbase = guard - (kMagicBits << 2) - (kSlab ? ((uint32_t)tp.slot_base << 2) : 0u);
-    const uint32_t g2base = guard + ((uint32_t)tp.tile_bins << 2);
     const long long n_items = (tp.total_centres + kItemCentres - 1) / kItemCentres;
 
     // work queue: a CTA first takes one of its own `cta_item_cap` tickets, then a global item
@@ -251,11 +302,14 @@ tiled_triplet_kernel(TriParams tp) {
             ksn = sp[0]; Kn = sp[1];              // entries at or beyond the slab's end are not needed
         }
         float4 v0n = tp.nbv[c * tp.max_nb + lane], v1n = tp.nbv[c * tp.max_nb + 32 + lane];
+        uint32_t j0n = tp.nbj[c * tp.max_nb + lane], j1n = tp.nbj[c * tp.max_nb + 32 + lane];
         bool more = true;
         while (more) {
             const int32_t K = Kn, ks = ksn;
             const float4 v0 = v0n, v1 = v1n;
+            const uint32_t j0 = j0n, j1 = j1n;
             const float4* __restrict__ lv = tp.nbv + c * tp.max_nb;
+            const uint32_t* __restrict__ lj = tp.nbj + c * tp.max_nb;
             // ---- advance and prefetch the next centre ------------------------------------------
             ++c;
             if (c >= c_end) {
@@ -272,25 +326,41 @@ tiled_triplet_kernel(TriParams tp) {
                 } else Kn = tp.nbcount[c];
                 v0n = tp.nbv[c * tp.max_nb + lane];
                 v1n = tp.nbv[c * tp.max_nb + 32 + lane];
+                j0n = tp.nbj[c * tp.max_nb + lane];
+                j1n = tp.nbj[c * tp.max_nb + 32 + lane];
             }
-            if (K < 2 || (kSlab && ks >= K)) {
-                if (K == 1 && ks == 0)           // a single neighbour: no pair, but one g2 count
-                    red_shared_add(lane == 0 ? g2base + ((uint32_t)__float_as_int(v0.w) << 2) : guard, 1u);
+            if (K < 2 || (kSlab && ks >= K)) continue;
+
+            if (!kSlab && K <= kWinEntries) {
+                // ---- the whole list fits the window: entries 0..31 = block A, 32..K-1 = block B ----
+                __syncwarp();
+                win[lane] = v0; win[32 + lane] = v1;
+                winJ[lane] = cbase + j0; winJ[32 + lane] = cbase + j1;
+                __syncwarp();
+                const JQuad qa = load_jquad(win, winJ, lane);
+                block_pairs(tp, win, winJ, guard, lane, min(K, 32), qa);
+                const int32_t kb = K - 32;
+                if (kb > 0) {
+                    rect32(tp, win + 32, guard, lane, 0, kb, qa);
+                    if (kb <= 16) {
+                        if (kb >= 2) triangle16(tp, win + 32, winJ + 32, guard, lane, kb);
+                    } else {                               // B = 16 + m entries
+                        triangle16(tp, win + 32, winJ + 32, guard, lane, 16);
+                        rect16(tp, win + 32, winJ + 32, win + 48, guard, lane, kb - 16);
+                        if (kb >= 18) triangle16(tp, win + 48, winJ + 48, guard, lane, kb - 16);
+                    }
+                }
                 continue;
             }
 
-            // ---- all unordered pairs of this centre's K neighbours ------------------------------
+            // ---- long lists and slab passes: a 32-block of j entries against all later k ----------
+            float4* winB = win + 32;
             const int32_t nchunks = (K + 31) >> 5;
             for (int32_t r = 0; r < nchunks; ++r) {
                 const int32_t jidx = (r << 5) + lane;
                 float4 jraw = r == 0 ? v0 : v1;
-                if (r >= 2 && jidx < K) jraw = lv[jidx];
-                const bool jvalid = jidx < K;
-                const int32_t aj = jvalid ? __float_as_int(jraw.w) : 0;
-                JSide own;
-                own.x = jvalid ? jraw.x : 0.f; own.y = jvalid ? jraw.y : 0.f; own.z = jvalid ? jraw.z : 0.f;
-                own.J = cbase + (uint32_t)tab_j[aj];
-                red_shared_add(jvalid && (!kSlab || jidx >= ks) ? g2base + ((uint32_t)aj << 2) : guard, 1u);
+                uint32_t jj = r == 0 ? j0 : j1;
+                if (r >= 2 && jidx < K) { jraw = lv[jidx]; jj = lj[jidx]; }
                 // prefetch the first rectangular window while the triangle runs
                 // (slab passes: the first k block is the one that holds list position ks)
                 const int32_t q_first = kSlab ? max(r + 1, ks >> 5) : r + 1;
@@ -299,73 +369,61 @@ tiled_triplet_kernel(TriParams tp) {
 
                 // ---- triangle: both members in this 32-block -------------------------------------
                 __syncwarp();
-                winA[lane] = make_float4(own.x, own.y, own.z, tab_addend[aj]);
-                winJ[lane] = own.J;
+                win[lane] = jraw;
+                winJ[lane] = cbase + jj;
                 __syncwarp();
                 const int32_t kt = min(32, K - (r << 5));
+                const JQuad qa = load_jquad(win, winJ, lane);
                 if (kSlab && ks > (r << 5)) {          // k members bounded below inside this block
-                    if (ks < (r << 5) + kt) triangle_from(tp, winA, guard, lane, ks - (r << 5), kt, own);
-                } else if (kt == 32) triangle32<true>(tp, winA, winJ, guard, lane, kt, own);
-                else if (kt > 16) triangle32<false>(tp, winA, winJ, guard, lane, kt, own);
-                else if (kt >= 2) triangle16(tp, winA, winJ, guard, lane, kt);
+                    if (ks < (r << 5) + kt) {
+                        JSide own;
+                        own.x = jraw.x; own.y = jraw.y; own.z = jraw.z; own.J = cbase + jj;
+                        triangle_from(tp, win, guard, lane, ks - (r << 5), kt, own);
+                    }
+                } else block_pairs(tp, win, winJ, guard, lane, kt, qa);
                 if (r + 1 == nchunks) break;
 
-                // ---- rectangles: k in later 32-blocks; this block is full, 2 j x 2 k per lane ----
-                const int kg = lane >> 4;
-                const JSide ja = load_jside(winA, winJ, lane & 15), jb = load_jside(winA, winJ, (lane & 15) + 16);
+                // ---- rectangles: k in later 32-blocks; this block is full ---------------------------
                 for (int32_t q = q_first; q < nchunks; ++q) {
-                    const bool kvalid = (q << 5) + lane < K;
-                    const int32_t ak = kvalid ? __float_as_int(nextv.w) : 0;
                     __syncwarp();
-                    winB[lane] = make_float4(kvalid ? nextv.x : 0.f, kvalid ? nextv.y : 0.f,
-                                             kvalid ? nextv.z : 0.f, tab_addend[ak]);
+                    winB[lane] = nextv;
                     __syncwarp();
                     if (q + 1 < nchunks && ((q + 1) << 5) + lane < K) nextv = lv[((q + 1) << 5) + lane];
                     const int32_t kc = min(32, K - (q << 5));
                     const int32_t klo = kSlab ? max(0, ks - (q << 5)) : 0;
-                    for (int32_t k0i = klo & ~3; k0i < kc; k0i += 4) {     // k = k0i + kg and k0i + kg + 2
-                        const int32_t kidx = k0i + kg;
-                        const float4 k0 = winB[kidx], k1 = winB[kidx + 2];
-                        if (k0i + 4 <= kc && (!kSlab || k0i >= klo))
-                            four_pairs<false>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, true, true, true, true);
-                        else {
-                            const bool pa = kidx < kc && kidx >= klo, pb = kidx + 2 < kc && kidx + 2 >= klo;
-                            four_pairs<true>(tp, guard, k0, k0, k1, k1, ja, jb, ja, jb, pa, pa, pb, pb);
-                        }
-                    }
+                    rect32(tp, winB, guard, lane, klo, kc, qa);
                 }
             }
         }
     }
     __syncthreads();
     unsigned long long* out = tp.scratch + (size_t)blockIdx.x * (size_t)tp.scratch_stride;
-    for (int32_t i = 1 + threadIdx.x; i < tp.tile_bins; i += blockDim.x) {
+    for (int32_t i = 1 + threadIdx.x; i < tp.tile_bins - 1; i += blockDim.x) {
         const uint32_t v = tile[i];
         if (v) out[i] += v;
     }
-    for (int32_t a = threadIdx.x; a < tp.n_r; a += blockDim.x) {
-        const uint32_t v = tile[tp.tile_bins + a];
-        if (v) out[tp.g2_out + a] += v;
-    }
+    // the two guard slots hold only the dummy adds of lanes without a pair; the top one must stay
+    // empty: anything there is reported through the unmapped slot 0 of the partial tile (stats[3])
+    if (threadIdx.x == 0 && tile[tp.tile_bins - 1] != 0) out[kSlab ? -(long long)tp.slot_base : 0] += tile[tp.tile_bins - 1];
 }
 
 // Mirror the per-CTA partial tiles into the uint64 histogram (step a5) and clear them.
 // One thread per slot; each slot maps to a unique (a, b, c), so no atomics are needed.
+// stats[3] counts what must never happen: counts in a slot no (a, b, c) maps to, or in a
+// top guard slot (slot 0 of a CTA's partial tile, see above).
 __global__ void __launch_bounds__(256)
 merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restrict__ slot_map,
              int32_t tile_bins, int32_t grid, int32_t n_r, int32_t n_t,
-             unsigned long long* __restrict__ counts, unsigned long long* __restrict__ counts2,
-             unsigned long long* __restrict__ stats) {
+             unsigned long long* __restrict__ counts, unsigned long long* __restrict__ stats) {
     const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= tile_bins + n_r) return;
+    if (i >= tile_bins) return;
     unsigned long long v = 0;
     for (int32_t gidx = 0; gidx < grid; ++gidx) {
-        unsigned long long* p = scratch + (size_t)gidx * (tile_bins + n_r) + i;
+        unsigned long long* p = scratch + (size_t)gidx * tile_bins + i;
         const unsigned long long x = *p;
         if (x) { v += x; *p = 0; }
     }
     if (v == 0) return;
-    if (i >= tile_bins) { counts2[i - tile_bins] += v; return; }      // g2 slots
     const uint32_t m = slot_map[i];
     if (m == 0xFFFFFFFFu) { atomicAdd(stats + 3, v); return; }      // must never happen
     const int32_t a = (int32_t)(m >> 21), b = (int32_t)((m >> 11) & 1023), c = (int32_t)(m & 2047);
@@ -378,7 +436,8 @@ merge_kernel(unsigned long long* __restrict__ scratch, const uint32_t* __restric
 }
 
 inline size_t tri_smem_bytes(int64_t tile_bins, int warps, int32_t n_r) {
-    return (((size_t)(tile_bins + n_r) * 4 + 15) & ~size_t(15)) + (size_t)warps * (64 * 16 + 32 * 4) + (size_t)n_r * 8;
+    (void)n_r;
+    return (((size_t)tile_bins * 4 + 15) & ~size_t(15)) + (size_t)warps * kWinBytes;
 }
 
 }  // namespace g3
