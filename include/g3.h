@@ -208,15 +208,6 @@ G3_API int g3_bin_volumes(const g3_plan *p, double *h_volumes);
 G3_API int g3_msd(const double *d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
                   int64_t max_lag, uint64_t *d_sums, double *d_msd, void *stream);
 
-/* Measure, on the current device, one of the two ceilings the triplet kernel's roofline is
- * quoted against: which = 0, shared-memory atomic increments per
- * second over the whole GPU for pseudo-random slots of a `slots`-word tile (bank conflicts
- * included; one CTA of 20 full warps per SM, like the triplet kernel); which = 1, issued FP32
- * thread instructions per second (slots ignored).  `iters` operations per thread.  Runs twice
- * (warm-up, then timed with CUDA events on `stream`), synchronises, writes *h_rate (host).
- * No result of the g(3) path depends on it.  Errors: G3_EINVAL, G3_ECUDA.                    */
-G3_API int g3_microbench(int32_t which, int64_t slots, int64_t iters, double *h_rate, void *stream);
-
 /* Zero the histogram, frame count and error state; keep all buffers.                */
 G3_API int g3_plan_reset(g3_plan *p, void *stream);
 

@@ -568,6 +568,17 @@ int64_t g3o_msd(const double *pos, int64_t n_frames, int64_t n, double box, int6
     return 0;
 }
 
+/* Thread count of the OpenMP loops (bench.py's single-thread figure: the analogue of the paper's
+ * serial code).  No effect on any result: the sums are integers. */
+void g3o_set_num_threads(int32_t n)
+{
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int32_t g3o_num_threads(void)
 {
 #ifdef _OPENMP

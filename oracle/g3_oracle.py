@@ -50,6 +50,8 @@ def _load() -> C.CDLL:
         _lib.g3o_msd.argtypes = [f64p, C.c_int64, C.c_int64, C.c_double, C.c_int64, u64p, f64p]
         _lib.g3o_msd.restype = C.c_int64
         _lib.g3o_num_threads.restype = C.c_int32
+        _lib.g3o_set_num_threads.argtypes = [C.c_int32]
+        _lib.g3o_set_num_threads.restype = None
         for fn in (_lib.g3o_thresholds, _lib.g3o_quantise, _lib.g3o_accumulate, _lib.g3o_volumes,
                    _lib.g3o_normalise):
             fn.restype = None
@@ -62,6 +64,11 @@ def _p(a: np.ndarray, ty):
 
 def num_threads() -> int:
     return int(_load().g3o_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of the following calls (results do not depend on it)."""
+    _load().g3o_set_num_threads(int(n))
 
 
 def thresholds(box: float, r_max: float, n_r: int, n_t: int) -> Tuple[np.ndarray, np.ndarray]:

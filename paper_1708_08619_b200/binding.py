@@ -24,7 +24,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_microbench", "g3_msd", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_msd", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -64,7 +64,6 @@ def load() -> C.CDLL:
     lib.g3_finalize_qtet.argtypes = [vp, vp, vp, vp]
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
-    lib.g3_microbench.argtypes = [i32, i64, i64, C.POINTER(f64), vp]
     lib.g3_msd.argtypes = [vp, i64, i64, i64, f64, i64, vp, vp, vp]
     lib.g3_plan_reset.argtypes = [vp, vp]
     lib.g3_plan_destroy.argtypes = [vp]
@@ -95,10 +94,28 @@ def _stream_ptr(stream) -> int:
     return int(stream.cuda_stream)
 
 
+BENCH_LIB_PATH = os.path.join(_HERE, "libg3bench.so")
+BENCH_EXPORTS = ["g3_microbench"]
+_bench_lib: Optional[C.CDLL] = None
+
+
+def load_bench() -> C.CDLL:
+    """dlopen libg3bench.so (include/g3_bench.h): bench.py's measurement aid, not the product."""
+    global _bench_lib
+    if _bench_lib is None:
+        if not os.path.exists(BENCH_LIB_PATH):
+            raise RuntimeError(f"{BENCH_LIB_PATH} is missing: run `python -m paper_1708_08619_b200.build`")
+        lib = C.CDLL(BENCH_LIB_PATH)
+        lib.g3_microbench.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.POINTER(C.c_double), C.c_void_p]
+        lib.g3_microbench.restype = C.c_int
+        _bench_lib = lib
+    return _bench_lib
+
+
 def microbench(which: int, slots: int = 50776, iters: int = 1 << 14, stream=None) -> float:
     """g3_microbench: 0 = shared-atomic increments/s (random slots), 1 = FP32 thread instr/s."""
     rate = C.c_double()
-    _check(load().g3_microbench(int(which), int(slots), int(iters), C.byref(rate), _stream_ptr(stream)),
+    _check(load_bench().g3_microbench(int(which), int(slots), int(iters), C.byref(rate), _stream_ptr(stream)),
            "g3_microbench")
     return float(rate.value)
 

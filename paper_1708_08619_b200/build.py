@@ -9,6 +9,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libg3.so")
+BENCH_LIB = os.path.join(_HERE, "libg3bench.so")      # measurement aid of bench.py (include/g3_bench.h)
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -31,17 +32,23 @@ def sources():
 
 
 def needs_build() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(BENCH_LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = glob.glob(os.path.join(CSRC, "*")) + [os.path.join(_HERE, "..", "include", "g3.h")]
+    deps = glob.glob(os.path.join(CSRC, "*")) + glob.glob(os.path.join(CSRC, "bench", "*")) + \
+        glob.glob(os.path.join(_HERE, "..", "include", "*.h"))
     return any(os.path.getmtime(d) > t for d in deps)
+
+
+def bench_sources():
+    return sorted(glob.glob(os.path.join(CSRC, "bench", "*.cu")))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", LIB]
-        subprocess.run(cmd, check=True)
+        extra = ["-Xptxas", "-v"] if verbose else []
+        subprocess.run([_nvcc()] + NVCC_FLAGS + extra + sources() + ["-o", LIB], check=True)
+        subprocess.run([_nvcc()] + NVCC_FLAGS + extra + bench_sources() + ["-o", BENCH_LIB], check=True)
     return LIB
 
 

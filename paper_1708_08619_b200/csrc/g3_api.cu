@@ -17,7 +17,6 @@
 
 #include "g3_cells.cuh"
 #include "g3_generic.cuh"
-#include "g3_microbench.cuh"
 #include "g3_msd.cuh"
 #include "g3_plan.h"
 #include "g3_qtet.cuh"
@@ -68,6 +67,7 @@ void free_buffers(g3_plan* p) {
     cudaFree(p->d_cell_count); p->d_cell_count = nullptr;
     cudaFree(p->d_cell_start); p->d_cell_start = nullptr;
     cudaFree(p->d_sorted); p->d_sorted = nullptr;
+    cudaFree(p->d_sortedf); p->d_sortedf = nullptr;
     cudaFree(p->d_h2d); p->d_h2d = nullptr;
     cudaFree(p->d_qtet); p->d_qtet = nullptr;
     cudaFree(p->d_qtet_stats); p->d_qtet_stats = nullptr;
@@ -121,8 +121,7 @@ int configure(g3_plan* p) {
     if (p->kernel == 1) {
         size_t smem = generic_smem_bytes(p->bins.n_r, p->bins.n_t, p->max_nb, kGenericWarps);
         if (smem > (size_t)p->smem_optin) return G3_EINVAL;   // neighbour capacity too large
-        G3_CUDA(cudaFuncSetAttribute(generic_triplet_kernel<kGenericWarps>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        G3_CUDA(allow_max_dynamic_smem(generic_triplet_kernel<kGenericWarps>, p->smem_optin));
     } else {
         int rc = tiled_configure(p);
         if (rc != G3_OK) return rc;
@@ -134,21 +133,20 @@ int configure(g3_plan* p) {
     G3_CUDA(cudaMalloc(&p->d_cell_count, sizeof(int32_t) * B * nc3));
     G3_CUDA(cudaMalloc(&p->d_cell_start, sizeof(int32_t) * B * (nc3 + 1)));
     G3_CUDA(cudaMalloc(&p->d_sorted, sizeof(int4) * B * n));
+    G3_CUDA(cudaMalloc(&p->d_sortedf, sizeof(float4) * B * n));
     G3_CUDA(cudaMemset(p->d_cell_count, 0, sizeof(int32_t) * B * nc3));
     if (p->qtet_bins > 0) {
         G3_CUDA(cudaMalloc(&p->d_qtet, sizeof(unsigned long long) * p->qtet_bins));
         G3_CUDA(cudaMalloc(&p->d_qtet_stats, sizeof(unsigned long long) * 2));
         G3_CUDA(cudaMemset(p->d_qtet, 0, sizeof(unsigned long long) * p->qtet_bins));
         G3_CUDA(cudaMemset(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2));
-        G3_CUDA(cudaFuncSetAttribute(qtet_kernel<kQtetWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(sizeof(unsigned int) * p->qtet_bins)));
-        G3_CUDA(cudaFuncSetAttribute(qtet_redo_kernel<kQtetWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(sizeof(unsigned int) * p->qtet_bins)));
+        G3_CUDA(allow_max_dynamic_smem(qtet_kernel<kQtetWarps>, p->smem_optin));
+        G3_CUDA(allow_max_dynamic_smem(qtet_redo_kernel<kQtetWarps>, p->smem_optin));
         if (p->ncell > 1 && B * n < (int64_t(1) << 31)) {   // fast path: 27 cells staged per CTA
             p->qtet_stage_cap = tiled_stage_cap(p);
             const size_t smem = qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins);
             if (smem <= (size_t)p->smem_optin) {
-                G3_CUDA(cudaFuncSetAttribute(qtet_cell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                G3_CUDA(allow_max_dynamic_smem(qtet_cell_kernel, p->smem_optin));
                 G3_CUDA(cudaMalloc(&p->d_qtet_redo, sizeof(int32_t) * (size_t)(B * n + 1)));
                 const int32_t nc = p->ncell;
                 std::vector<int4> origin((size_t)nc3);
@@ -176,11 +174,11 @@ int flush(g3_plan* p, cudaStream_t st) {
     const long long total = (long long)F * n;
     cell_scan_kernel<<<F, 1024, 0, st>>>(p->d_cell_count, p->d_cell_start, nc3);
     cell_scatter_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(
-        p->d_staged, p->d_slot, p->d_cell_start, n, F, nc3, p->d_sorted);
+        p->d_staged, p->d_slot, p->d_cell_start, n, F, nc3, p->d_sorted, p->d_sortedf);
     p->launches += 2;
     G3_CUDA(cudaMemsetAsync(p->d_cell_count, 0, sizeof(int32_t) * (size_t)F * nc3, st));
 
-    FrameBatch fb{n, F, p->ncell, nc3, p->d_sorted, p->d_cell_start};
+    FrameBatch fb{n, F, p->ncell, nc3, p->d_sorted, p->d_sortedf, p->d_cell_start};
     BinSpec bs{p->bins.n_r, p->bins.n_t, p->d_T_r, p->d_T_t, p->T_r.back()};
     if (p->kernel == 1) {
         size_t smem = generic_smem_bytes(bs.n_r, bs.n_t, p->max_nb, kGenericWarps);
@@ -566,44 +564,6 @@ int g3_finalize_host(g3_plan* p, uint64_t* h_counts, double* h_g3, uint64_t* h_s
     }
     if (d_g3) cudaFreeAsync(d_g3, st);
     return rc;
-}
-
-int g3_microbench(int32_t which, int64_t slots, int64_t iters, double* h_rate, void* stream) {
-    if (!h_rate || iters < 8 || iters > (int64_t(1) << 30) || which < 0 || which > 1) return G3_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    int dev = 0;
-    cudaDeviceProp prop;
-    G3_CUDA(cudaGetDevice(&dev));
-    G3_CUDA(cudaGetDeviceProperties(&prop, dev));
-    if (prop.major < 10) return G3_ECUDA;
-    const int grid = prop.multiProcessorCount;
-    const int32_t it = (int32_t)((iters + 127) / 128 * 128);
-    unsigned int* d_sink = nullptr;
-    G3_CUDA(cudaMalloc(&d_sink, 16));
-    cudaEvent_t e0, e1;
-    G3_CUDA(cudaEventCreate(&e0));
-    G3_CUDA(cudaEventCreate(&e1));
-    int rc = G3_OK;
-    float ms = 0.f;
-    for (int rep = 0; rep < 2 && rc == G3_OK; ++rep) {          // first pass warms up
-        cudaEventRecord(e0, st);
-        if (which == 0) {
-            if (slots < 32 || slots * 4 > (int64_t)prop.sharedMemPerBlockOptin) { rc = G3_EINVAL; break; }
-            cudaFuncSetAttribute(mb_shared_atomic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)(slots * 4));
-            mb_shared_atomic_kernel<<<grid, kMbThreads, (size_t)slots * 4, st>>>((int32_t)slots, it, d_sink);
-        } else {
-            mb_issue_kernel<<<grid, kMbThreads, 0, st>>>(it, 1.0f, reinterpret_cast<float*>(d_sink));
-        }
-        cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = G3_ECUDA;
-        else cudaEventElapsedTime(&ms, e0, e1);
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_sink);
-    if (rc != G3_OK) return rc;
-    // thread-level operations per second over the whole GPU (loop overhead not counted)
-    *h_rate = (double)grid * kMbThreads * (double)it / ((double)ms * 1e-3);
-    return G3_OK;
 }
 
 int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,

@@ -90,13 +90,14 @@ cell_scan_kernel(const int32_t* __restrict__ cell_count, int32_t* __restrict__ c
 __global__ void __launch_bounds__(256)
 cell_scatter_kernel(const int4* __restrict__ staged, const int32_t* __restrict__ slot,
                     const int32_t* __restrict__ cell_start, int32_t n, int32_t n_frames,
-                    int32_t ncell3, int4* __restrict__ sorted) {
+                    int32_t ncell3, int4* __restrict__ sorted, float4* __restrict__ sortedf) {
     long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (long long)n_frames * n) return;
     int32_t f = (int32_t)(g / n);
     int4 v = staged[g];
     int32_t dst = cell_start[(long long)f * (ncell3 + 1) + v.w] + slot[g];
     sorted[(long long)f * n + dst] = v;
+    sortedf[(long long)f * n + dst] = make_float4((float)v.x, (float)v.y, (float)v.z, 0.f);
 }
 
 }  // namespace g3

@@ -21,6 +21,7 @@ struct FrameBatch {
     int32_t ncell;             // cells per edge (1 = no cell grid: every particle is a candidate)
     int32_t ncell3;
     const int4* sorted;        // [frames][n]  (x, y, z, cell id), cell-major order
+    const float4* sortedf;     // [frames][n]  the same coordinates as fp32 (exact: < 2^20), w = 0
     const int32_t* cell_start; // [frames][ncell3 + 1]
 };
 
@@ -30,6 +31,18 @@ struct BinSpec {
     const unsigned long long* T_t;  // device, [n_t + 1]
     unsigned long long cut2;        // T_r[n_r]
 };
+
+// The dynamic shared-memory limit of a kernel is state of the whole context, shared by every
+// plan: it is always set to the device maximum (opt-in limit minus the kernel's static shared
+// memory), never to one plan's own size, so plans of different shape cannot disturb each other.
+template <class Kernel>
+inline cudaError_t allow_max_dynamic_smem(Kernel kernel, int smem_optin) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                smem_optin - (int)fa.sharedSizeBytes);
+}
 
 }  // namespace g3
 
@@ -81,6 +94,7 @@ struct g3_plan {
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]
     int32_t* d_cell_start = nullptr;         // [batch][ncell3 + 1]
     int4* d_sorted = nullptr;                // [batch][n]
+    float4* d_sortedf = nullptr;             // [batch][n] fp32 copy of d_sorted (TMA source of the neighbour kernel)
     double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
     cudaEvent_t h2d_done[2] = {nullptr, nullptr};   // copy of a staging half finished (copy stream)
     cudaEvent_t h2d_free[2] = {nullptr, nullptr};   // staging half consumed (caller's stream)

@@ -37,9 +37,11 @@ struct TiledState {
     int32_t* d_nbcount = nullptr;              // [batch][n]
     unsigned int* d_work = nullptr;            // work-queue counter
     int4* d_cell_origin = nullptr;             // [ncell3] cell centres on the grid
+    float4* d_crowd = nullptr;                 // [nb_grid][kNbWarps][max_nb] lists of the neighbour kernel's crowded path
     // launch configuration
     int tri_warps = 16;
     int grid = 0;
+    int nb_grid = 0;                           // persistent CTAs of neighbour_cell_kernel
     size_t tri_smem = 0, nb_smem = 0;
     int32_t stage_cap = 0;
     uint32_t cta_item_cap = 0;                 // work items one CTA may take per launch
@@ -123,9 +125,9 @@ inline void build_layout(const g3_plan* p, TiledState& ts) {
 // host side
 inline int32_t tiled_stage_cap(const g3_plan* p) {
     if (p->ncell == 1) return (int32_t)((p->n + 63) / 64 * 64);
-    // twice the mean occupancy of 27 cells; more crowded neighbourhoods are read from global
+    // 1.5 x the mean occupancy of 27 cells; more crowded neighbourhoods are read from global
     const double per27 = 27.0 * (double)p->n / ((double)p->ncell * p->ncell * p->ncell);
-    const int64_t cap = (int64_t)(2.0 * per27) + 96;
+    const int64_t cap = (int64_t)(1.5 * per27) + 96;
     return (int32_t)((cap + 63) / 64 * 64);
 }
 
@@ -162,7 +164,8 @@ inline int32_t tiled_select(g3_plan* p) {
     if (p->max_nb > (1 << 16)) return 1;
     TiledState ts;
     if (!tiled_plan_slabs(p, ts)) return 1;
-    if (nb_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r) > (size_t)p->smem_optin) return 1;
+    if ((p->ncell == 1 ? nb_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r)
+                       : nb_cell_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r, kNbStages)) + 1024 > (size_t)p->smem_optin) return 1;   // + static shared
     if (p->ncell == 1 && p->n > 8192) return 1;
     return 2;
 }
@@ -172,7 +175,7 @@ inline void tiled_free(g3_plan* p) {
     if (!ts) return;
     cudaFree(ts->d_addend); cudaFree(ts->d_jconst); cudaFree(ts->d_slot_map); cudaFree(ts->d_scratch);
     cudaFree(ts->d_nbv); cudaFree(ts->d_nbj); cudaFree(ts->d_nbcount); cudaFree(ts->d_work); cudaFree(ts->d_cell_origin);
-    cudaFree(ts->d_slab_shell); cudaFree(ts->d_slabpos);
+    cudaFree(ts->d_slab_shell); cudaFree(ts->d_slabpos); cudaFree(ts->d_crowd);
     delete ts;
     p->tiled = nullptr;
 }
@@ -187,11 +190,9 @@ inline void tiled_free(g3_plan* p) {
     } while (0)
 
 template <int kWarps>
-inline int tiled_set_attr(size_t smem) {
-    G3T_CUDA(cudaFuncSetAttribute(tiled_triplet_kernel<kWarps, false>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    G3T_CUDA(cudaFuncSetAttribute(tiled_triplet_kernel<kWarps, true>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+inline int tiled_set_attr(int smem_optin) {
+    G3T_CUDA(allow_max_dynamic_smem(tiled_triplet_kernel<kWarps, false>, smem_optin));
+    G3T_CUDA(allow_max_dynamic_smem(tiled_triplet_kernel<kWarps, true>, smem_optin));
     return G3_OK;
 }
 
@@ -230,7 +231,8 @@ inline int tiled_configure(g3_plan* p) {
     ts->tri_warps = tiled_warps(p, ts->slab_bins_max);
     ts->tri_smem = tri_smem_bytes(ts->slab_bins_max, ts->tri_warps, n_r);
     ts->stage_cap = tiled_stage_cap(p);
-    ts->nb_smem = nb_smem_bytes(ts->stage_cap, p->max_nb, n_r);
+    ts->nb_smem = p->ncell == 1 ? nb_smem_bytes(ts->stage_cap, p->max_nb, n_r)
+                                : nb_cell_smem_bytes(ts->stage_cap, p->max_nb, n_r, kNbStages);
 
     std::vector<float> addend(n_r);
     std::vector<int32_t> jconst(n_r);
@@ -285,14 +287,22 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMemcpy(ts->d_slot_map, slot_map.data(), sizeof(uint32_t) * ts->tile_bins, cudaMemcpyHostToDevice));
     G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
     G3T_CUDA(cudaMemset(ts->d_nbv, 0, sizeof(float4) * (per_frame_entries * B + 64)));
-    G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
-    G3T_CUDA(cudaFuncSetAttribute(neighbour_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ts->nb_smem));
+    if (p->ncell == 1) {
+        G3T_CUDA(allow_max_dynamic_smem(neighbour_kernel<true>, p->smem_optin));
+    } else {
+        auto kern = neighbour_cell_kernel<kNbStages>;
+        G3T_CUDA(allow_max_dynamic_smem(kern, p->smem_optin));
+        int per_sm = 0;      // persistent: exactly the CTAs that are resident together
+        G3T_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, (kNbWarps + 1) * 32, ts->nb_smem));
+        ts->nb_grid = p->sm_count * std::max(per_sm, 1);
+        G3T_CUDA(cudaMalloc(&ts->d_crowd, sizeof(float4) * (size_t)ts->nb_grid * kNbWarps * p->max_nb));
+    }
     switch (ts->tri_warps) {
-        case 24: return tiled_set_attr<24>(ts->tri_smem);
-        case 20: return tiled_set_attr<20>(ts->tri_smem);
-        case 12: return tiled_set_attr<12>(ts->tri_smem);
-        case 16: return tiled_set_attr<16>(ts->tri_smem);
-        default: return tiled_set_attr<8>(ts->tri_smem);
+        case 24: return tiled_set_attr<24>(p->smem_optin);
+        case 20: return tiled_set_attr<20>(p->smem_optin);
+        case 12: return tiled_set_attr<12>(p->smem_optin);
+        case 16: return tiled_set_attr<16>(p->smem_optin);
+        default: return tiled_set_attr<8>(p->smem_optin);
     }
 }
 
@@ -324,7 +334,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     np.T_r = bs.T_r;
     np.cell_origin = ts->d_cell_origin;
     np.nbv = ts->d_nbv; np.nbj = ts->d_nbj; np.addend = ts->d_addend; np.jconst = ts->d_jconst; np.nbcount = ts->d_nbcount; np.stats = p->d_stats; np.counts2 = p->d_counts2;
-    np.n_slabs = ts->n_slabs; np.slab_shell = ts->d_slab_shell; np.slabpos = ts->d_slabpos;
+    np.n_slabs = ts->n_slabs; np.slab_shell = ts->d_slab_shell; np.slabpos = ts->d_slabpos; np.crowd_scratch = ts->d_crowd;
     G3T_CUDA(cudaMemsetAsync(ts->d_work, 0, sizeof(unsigned int), st));
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     if (p->timing) {
@@ -342,8 +352,9 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
         dim3 grid((unsigned)((fb.n + 63) / 64), (unsigned)fb.n_frames);
         neighbour_kernel<true><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
     } else {
-        dim3 grid((unsigned)fb.ncell3, (unsigned)fb.n_frames);
-        neighbour_kernel<false><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
+        const long long items = (long long)fb.ncell3 * fb.n_frames;
+        auto kern = neighbour_cell_kernel<kNbStages>;
+        kern<<<(unsigned)std::min<long long>(items, ts->nb_grid), (kNbWarps + 1) * 32, ts->nb_smem, st>>>(fb, np);
     }
     if (p->timing) G3T_CUDA(cudaEventRecord(ev[1], st));
     TriParams tp;

@@ -17,9 +17,9 @@ def lib():
     return g3.load()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "g3.h")).read()
-    return re.findall(r"G3_API\s+[\w\s\*]+?\b(g3_\w+)\s*\(", text)
+def declared_symbols(header="g3.h", macro="G3_API"):
+    text = open(os.path.join(ROOT, "include", header)).read()
+    return re.findall(macro + r"\s+[\w\s\*]+?\b(g3_\w+)\s*\(", text)
 
 
 def test_header_symbols_exported(lib):
@@ -32,6 +32,21 @@ def test_header_symbols_exported(lib):
 def test_binding_lists_the_same_names(lib):
     import paper_1708_08619_b200 as g3
     assert sorted(g3.EXPORTS) == sorted(declared_symbols())
+
+
+def test_every_header_has_its_library():
+    """every include/*.h is covered: g3.h -> libg3.so, g3_bench.h -> libg3bench.so (bench.py's
+    measurement aid, kept out of the product library)"""
+    import paper_1708_08619_b200 as g3
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["g3.h", "g3_bench.h"]
+    names = declared_symbols("g3_bench.h", "G3_BENCH_API")
+    assert sorted(names) == sorted(g3.BENCH_EXPORTS) == ["g3_microbench"]
+    blib = g3.load_bench()
+    for name in names:
+        assert hasattr(blib, name), name
+    assert not hasattr(g3.load(), "g3_microbench")          # not part of the product ABI
+    rate = ctypes.c_double()
+    assert blib.g3_microbench(7, 64, 1024, ctypes.byref(rate), None) == g3.G3_EINVAL
 
 
 def test_strerror_and_argument_errors(lib):

@@ -3,10 +3,11 @@ batch of 16 frames, event timing on, device and host entry points).
 
 * config 4 (headline, 500 frames) and configs 1-2: the oracle runs the whole trajectory; counts
   and statistics bit-exact, g3 to 1e-12.
-* configs 3 and 5 (1.5e10 / 6.7e10 triplets: minutes of oracle time): the whole trajectory goes
-  through the library once; the oracle computes SAMPLED frames one by one (the histogram is a
-  sum over frames) and the full run is tied to them by properties that hold
-  at any size: H(all frames) = sum of per-frame H; sum(H) + overflow = sum_i k_i (k_i - 1);
+* configs 3 and 5 (1.5e10 / 6.7e10 triplets: about one and five minutes of oracle time on 16
+  cores): the oracle also runs the WHOLE trajectory and the whole-run histogram, statistics and g3
+  are compared as above.  In addition the library's per-frame histograms are compared with the
+  oracle on sampled frames and tied to the whole run by properties that hold at any size:
+  H(all frames) = sum of per-frame H (PAPER.md:193, 356); sum(H) + overflow = sum_i k_i (k_i - 1);
   H[a][b][c] = H[b][a][c]; H = 0 where V_abc = 0; config 5 (ideal gas): g3 = (1-1/N)(1-2/N)
   within counting error.
 """
@@ -97,10 +98,11 @@ def test_full_trajectory_bit_exact(oracle_lib, g3, widx):
 
 
 @pytest.mark.parametrize("widx,sample", [(3, (0, 67, 133, 199)), (5, (0, 41, 99))])
-def test_full_trajectory_sampled(oracle_lib, g3, widx, sample):
+def test_full_trajectory_configs_3_and_5(oracle_lib, g3, widx, sample):
     import torch
     w = WORKLOADS[widx]
     ms = list(frame_iter(w, w.n_frames))
+    Ho_all, so_all = oracle_frames(oracle_lib, w, ms)          # the oracle over the whole trajectory
     d_pos = torch.from_numpy(grid_to_pos(np.stack(ms, axis=0), w.box)).cuda()
     with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, timing=True) as plan:
         assert plan.info(g3.G3_INFO_KERNEL) == 2
@@ -108,6 +110,8 @@ def test_full_trajectory_sampled(oracle_lib, g3, widx, sample):
         counts, G, stats = plan.finalize()
         H = counts.cpu().numpy().view(np.uint64).copy()
         G = G.cpu().numpy()
+        assert stats == so_all
+        assert np.array_equal(H, Ho_all), "whole-run histogram differs from the oracle"
         c2all, g2all = plan.finalize_g2()
         c2all = c2all.cpu().numpy().view(np.uint64).copy()
         g2all = g2all.cpu().numpy()

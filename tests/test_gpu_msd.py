@@ -57,6 +57,22 @@ def test_wide_range_and_128_bit_sums(oracle_lib, g3):
     assert int(so[1, 1]) > 0                                    # the high word is in use
 
 
+def test_range_edge_sum_of_squares_exceeds_63_bits(oracle_lib, g3):
+    """m = -(2^30 - 1) -> +(2^30 - 1) on all three axes: one squared displacement is
+    3 (2^31 - 2)^2 > 2^63 (readings M1, M2); the expected sum is a Python integer"""
+    e = (1 << 30) - 1
+    n = 67
+    m = np.zeros((3, n, 3), dtype=np.int64)
+    m[0] = -e
+    m[1] = e
+    m[2] = -e
+    so, _ = check(oracle_lib, g3, m, 1.0)
+    d2 = 3 * (2 * e) ** 2
+    assert d2 > (1 << 63)
+    want = [0, 2 * n * d2, 0]
+    assert [int(lo) + (int(hi) << 64) for lo, hi in so] == want
+
+
 def test_out_of_range_coordinate_is_an_error(g3):
     import torch
     pos = torch.zeros((2, 40, 3), dtype=torch.float64, device="cuda")

@@ -62,8 +62,6 @@ def check(oracle_lib, g3, pos, box, r_max, n_r, n_t, mode="cells", **opts):
     else:
         H2, _, _, i1 = run_gpu(g3, pos3[:1], box, r_max, n_r, n_t, **opts)
         assert np.array_equal(i1["counts2"], oracle_lib.g2_frame(oracle_lib.quantise(pos3[0], box), T_r))
-    if "kernel" in opts and opts["kernel"] in (1, 2) and opts.get("expect_kernel", True):
-        pass
     return H, stats, info
 
 
@@ -202,6 +200,62 @@ def test_capacity_error_is_reported(g3):
         with pytest.raises(g3.G3Error) as e:
             plan.finalize()
         assert e.value.code == g3.G3_ECAPACITY
+
+
+def test_capacity_error_through_the_tiled_path(g3):
+    """kernel 2: a clumped frame with far more than 64 neighbours per centre and max_neighbours = 64
+    (the tiled path's smallest capacity) must end in G3_ECAPACITY, on the staged and on the
+    crowded (unstaged) route of the neighbour kernel"""
+    import torch
+    rng = np.random.default_rng(17)
+    m = uniform_frame(6000, seed=3)
+    m[:400] = ((rng.integers(0, GRID // 64, size=(400, 3)) + GRID // 3) % GRID).astype(np.int32)   # a blob
+    pos = grid_to_pos(m, 10.0)
+    with g3.Plan(6000, 10.0, 1.2, 16, 16, max_neighbours=64, kernel=2) as plan:
+        assert plan.info(g3.G3_INFO_KERNEL) == 2 and plan.info(g3.G3_INFO_MAX_NEIGHBOURS) == 64
+        plan.accumulate_frames(torch.from_numpy(pos[None]).cuda())
+        with pytest.raises(g3.G3Error) as e:
+            plan.finalize()
+        assert e.value.code == g3.G3_ECAPACITY
+
+
+@pytest.mark.parametrize("warps", [8, 12, 16, 20, 24])
+def test_triplet_warps_option_full_config2(oracle_lib, g3, warps):
+    """G3_OPT_TRIPLET_WARPS instantiates one triplet kernel per value: the whole 100-frame config-2
+    trajectory through each, bit-exact against the oracle"""
+    w = WORKLOADS[2]
+    _, pos = frames(w, w.n_frames)
+    H, stats, _ = check(oracle_lib, g3, pos, w.box, w.r_max, w.n_r, w.n_t, kernel=2, triplet_warps=warps)
+    assert stats[0] == w.n_frames
+
+
+def test_two_live_plans_of_different_shape(oracle_lib, g3):
+    """distinct plans are independent (include/g3.h): interleave two plans whose kernels need
+    different amounts of dynamic shared memory (bins, neighbour capacity, q_tet histogram)"""
+    import torch
+    wa, wb = WORKLOADS[2], WORKLOADS[1]
+    _, pa = frames(wa, 4)
+    _, pb = frames(wb, 4)
+    da, db = torch.from_numpy(pa).cuda(), torch.from_numpy(pb).cuda()
+    with g3.Plan(wa.n, wa.box, wa.r_max, wa.n_r, wa.n_t, batch_frames=1, qtet_bins=300) as A, \
+         g3.Plan(wb.n, wb.box, wb.r_max, 8, 8, batch_frames=1, max_neighbours=96, qtet_bins=10) as B, \
+         g3.Plan(wa.n, wa.box, 0.9 * wa.r_max, 24, 48, batch_frames=2, kernel=1) as C:
+        for f in range(4):
+            A.accumulate_frame(da[f])
+            B.accumulate_frame(db[f])
+            C.accumulate_frame(da[f])
+        cb, _, sb = B.finalize(want_g3=False)
+        ca, _, sa = A.finalize(want_g3=False)
+        cc, _, sc = C.finalize(want_g3=False)
+        A.finalize_qtet()
+        B.finalize_qtet()
+    for (w, pos, n_r, n_t, r_max, c, st) in ((wa, pa, wa.n_r, wa.n_t, wa.r_max, ca, sa), (wb, pb, 8, 8, wb.r_max, cb, sb),
+                                             (wa, pa, 24, 48, 0.9 * wa.r_max, cc, sc)):
+        orc = oracle_lib.Oracle(w.n, w.box, r_max, n_r, n_t)
+        orc.accumulate(pos)
+        Ho, _, so = orc.finalize()
+        assert st == [int(v) for v in so]
+        assert np.array_equal(c.cpu().numpy().view(np.uint64), Ho)
 
 
 def test_normalize_merged_counts(oracle_lib, g3):

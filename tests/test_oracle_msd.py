@@ -63,6 +63,28 @@ def test_unwrapped_input_is_not_wrapped_and_128_bit_sums(oracle_lib):
         oracle_lib.msd(np.full((2, 1, 3), 1.0 * (1 << 11)), 1.0)       # 2^31 grid units
 
 
+def test_range_edge_sum_of_squares_exceeds_63_bits(oracle_lib):
+    """the corner of reading M1's range: m = -(2^30 - 1) -> +(2^30 - 1) on all three axes between
+    two frames, so one squared displacement is 3 (2^31 - 2)^2 > 2^63 (a signed 64-bit sum would
+    wrap); expected values from Python integers (readings M1, M2)"""
+    e = (1 << 30) - 1
+    n = 5
+    m = np.zeros((2, n, 3), dtype=np.int64)
+    m[0] = -e
+    m[1] = e
+    m[1, 3] = (e, -e, e)                       # mixed signs: displacement (2e, 0, 2e)
+    m[0, 3] = (-e, -e, -e)
+    want1 = (n - 1) * 3 * (2 * e) ** 2 + 2 * (2 * e) ** 2
+    assert 3 * (2 * e) ** 2 > (1 << 63)
+    sums, msd = oracle_lib.msd(grid_to_pos(m, 1.0), 1.0)
+    assert to128(sums) == [0, want1]
+    g = 1.0 / GRID
+    assert msd[1] == pytest.approx(want1 * g * g / n, rel=1e-15)
+    with pytest.raises(ValueError):            # one step further is outside the range
+        m[1, 0, 0] = e + 1
+        oracle_lib.msd(grid_to_pos(m, 1.0), 1.0)
+
+
 def test_invariances(oracle_lib):
     m = unwrapped_walk(50, 12, seed=5)
     box = 9.0
