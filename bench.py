@@ -12,15 +12,19 @@ second (frames/s is reported beside it).
 Prints ONE JSON line (rank 0).  `value` is device-timed with positions resident in HBM; `e2e` is
 the same step through the C ABI's host entry points (pinned host positions in, host results out,
 copies inside the timed region).  `roofline` and `cpu_baseline` are described in DESIGN.md 6.
-With --gpus N > 1 (torchrun) every rank processes its own trajectory of the same shape
-(frames are independent; "split the trajectory, merge the results",
-PAPER.md:356, 727): weak scaling, no data-path collective.
+With --gpus N > 1 every rank processes its own trajectory of the same shape (frames are
+independent, PAPER.md:193; "split the trajectory, merge the results", PAPER.md:356, 727): weak
+scaling, no data-path collective; --shard-one-trajectory instead splits the ONE seeded trajectory
+over the ranks with sharding.frame_shard (strong scaling).  Run as `python bench.py --gpus N`
+(no torchrun) it launches the N ranks itself through torch.distributed.run on 127.0.0.1.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import re
+import socket
 import statistics
 import subprocess
 import sys
@@ -40,10 +44,23 @@ UNIT = "triplets/s"
 WORKLOAD_INDEX = 4
 ALGO_INSTR_PER_TRIPLET = 12          # fixed algorithmic instruction count
 SM_LANES = 128                       # 4 schedulers x 32 lanes, one warp instruction per cycle each
-# dram__bytes_read.sum + dram__bytes_write.sum of one tiled_triplet_kernel launch (16 frames of
-# config 4) from the ncu --set full capture summarised in profiles/r1_triplet_kernel.md
-NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH = 598.884864e6 + 6.587904e6
-NCU_TRIPLET_FRAMES_PER_LAUNCH = 16
+ALGO_INSTR_PER_DISPLACEMENT = 9       # MSD: 3 subtractions, 3 multiply-adds, one 128-bit accumulate
+ALGO_INSTR_PER_QTET_ATOM = 210        # q_tet: exact keys + top-4 insertion of ~6 list-head entries (150) + Eq. 1 in fp64 (60)
+TRAFFIC_PROFILES = {"tiled_triplet_kernel": "r2_triplet_kernel.md", "neighbour_cell_kernel": "r2_neighbour_kernel.md"}
+
+
+def ncu_traffic(kernel: str, frames_per_launch: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, read from the ncu
+    summary committed under profiles/ (a line `traffic: dram_bytes_per_launch=<B> frames_per_launch=<F>`).
+    None when the file is missing or was captured at another batch size."""
+    path = os.path.join(ROOT, "profiles", TRAFFIC_PROFILES.get(kernel, ""))
+    try:
+        m = re.search(r"dram_bytes_per_launch=([0-9.eE+]+)\s+frames_per_launch=(\d+)", open(path).read())
+    except OSError:
+        return None, None
+    if not m or int(m.group(2)) != frames_per_launch:
+        return None, os.path.relpath(path, ROOT)
+    return float(m.group(1)), os.path.relpath(path, ROOT)
 
 
 def peaks():
@@ -110,26 +127,55 @@ def make_positions(w, n_frames: int, rank: int) -> np.ndarray:
     return grid_to_pos(np.stack(ms, axis=0), w.box)
 
 
-def cpu_baseline_leg(w, budget_s: float = 20.0):
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_baseline_leg(w, budget_s: float = 15.0):
     """The oracle as it stands (oracle/g3_oracle.c, cell-grid routine, OpenMP over centres) on a
-    bounded sample: whole frames of the same workload until ~budget_s of CPU time is spent."""
+    bounded sample of the same workload: whole frames (generated BEFORE the clock starts) until
+    ~budget_s of wall time on all host cores, then one frame on ONE thread (the analogue of the
+    paper's serial code)."""
     import oracle
     oracle.build()
     T_r, T_t = oracle.thresholds(w.box, w.r_max, w.n_r, w.n_t)
+    cores = oracle.num_threads()
+    # how many frames fit the budget: time one, then generate the sample up front
+    ms = list(frame_iter(w, 2))
     H = np.zeros((w.n_r, w.n_r, w.n_t), dtype=np.uint64)
     stats = np.zeros(3, dtype=np.uint64)
-    done, t0 = 0, time.perf_counter()
-    for m in frame_iter(w, w.n_frames):
+    t0 = time.perf_counter()
+    oracle.frame_cells(ms[0], T_r, T_t, H, stats)
+    per_frame = max(time.perf_counter() - t0, 1e-3)
+    n_sample = int(min(w.n_frames, max(2, budget_s / per_frame)))
+    ms = list(frame_iter(w, n_sample))
+    H[:] = 0
+    stats[:] = 0
+    t0 = time.perf_counter()
+    for m in ms:
         oracle.frame_cells(m, T_r, T_t, H, stats)
-        done += 1
-        if time.perf_counter() - t0 > budget_s:
-            break
     dt = time.perf_counter() - t0
-    triplets = (int(stats[1]) + 0) // 2
-    return {"value": triplets / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"first {done} frame(s) of {w.name} ({triplets} distinct triplets), "
-                      f"frame generation included, {dt:.1f} s wall",
-            "frames_per_s": done / dt}, done, dt, triplets
+    triplets = int(stats[1]) // 2
+    # single thread, one frame
+    oracle.set_num_threads(1)
+    H1 = np.zeros_like(H)
+    s1 = np.zeros(3, dtype=np.uint64)
+    t0 = time.perf_counter()
+    oracle.frame_cells(ms[0], T_r, T_t, H1, s1)
+    dt1 = time.perf_counter() - t0
+    oracle.set_num_threads(cores)
+    return {"value": triplets / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n_sample} frame(s) of {w.name} ({triplets} distinct triplets), frames generated "
+                      f"before the timed region, {dt:.1f} s wall",
+            "frames_per_s": n_sample / dt, "cpu_model": cpu_model(), "nproc": os.cpu_count(),
+            "single_thread": {"value": (int(s1[1]) // 2) / dt1, "unit": UNIT, "cores": 1,
+                              "sample": f"frame 0 of {w.name} ({int(s1[1]) // 2} distinct triplets), {dt1:.1f} s wall"}}
 
 
 def run_reference(args):
@@ -182,6 +228,45 @@ def run_reference(args):
     return 0
 
 
+def other_configs_leg(g3, torch, stream, peak_tinstr, steps: int):
+    """"also reported for the other four configs".  Whole path (a1..a6), device
+    resident, full BASELINE.json sizes, CUDA events; one warm-up step, then `steps` timed ones."""
+    out = {}
+    for widx in (1, 2, 3, 5):
+        w = WORKLOADS[widx]
+        try:
+            d_pos = torch.from_numpy(make_positions(w, w.n_frames, 0)).cuda()
+            with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t) as plan:
+                def step():
+                    plan.reset()
+                    plan.accumulate_frames(d_pos)
+                    return plan.finalize()
+                step()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(steps):
+                    _, _, stats = step()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / steps
+                triplets = (stats[1] + stats[2]) // 2
+                out[f"config{widx}"] = {
+                    "workload": f"{w.name}: N={w.n}, L={w.box}, r_max={w.r_max}, {w.n_r}x{w.n_r}x{w.n_t} bins, "
+                                f"{w.n_frames} frames",
+                    "value": triplets / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps,
+                    "frames_per_s": w.n_frames / (ms * 1e-3), "triplets_per_step": triplets,
+                    "whole_step_frac": triplets / (ms * 1e-3) * ALGO_INSTR_PER_TRIPLET / 1e12 / peak_tinstr,
+                    "batch_frames": plan.info(g3.G3_INFO_BATCH_FRAMES), "slabs": plan.info(g3.G3_INFO_SLABS),
+                    "kernel": plan.info(g3.G3_INFO_KERNEL), "cells_per_edge": plan.info(g3.G3_INFO_CELLS_PER_EDGE),
+                    "max_neighbours": plan.info(g3.G3_INFO_MAX_NEIGHBOURS)}
+            del d_pos
+            torch.cuda.empty_cache()
+        except Exception as e:  # the headline numbers stay valid
+            out[f"config{widx}"] = {"error": str(e)}
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -205,9 +290,15 @@ def run_ours(args):
     from paper_1708_08619_b200.sharding import merge_counts
 
     w = WORKLOADS[WORKLOAD_INDEX]
-    F = args.frames or w.n_frames
-    pos = make_positions(w, F, rank)                                  # fp64 [F, n, 3]
-    h_pos = torch.from_numpy(pos).pin_memory()
+    F_total = args.frames or w.n_frames
+    if args.shard_one_trajectory:                                     # strong scaling: one trajectory, frames split
+        from paper_1708_08619_b200.sharding import frame_shard
+        f0, f1 = frame_shard(F_total, rank, world)
+        pos = make_positions(w, F_total, 0)[f0:f1]
+    else:                                                             # weak scaling: one trajectory per rank
+        pos = make_positions(w, F_total, rank)                        # fp64 [F, n, 3]
+    F = pos.shape[0]
+    h_pos = torch.from_numpy(np.ascontiguousarray(pos)).pin_memory()
     d_pos = h_pos.cuda(non_blocking=True)
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream()
@@ -221,7 +312,11 @@ def run_ours(args):
         counts, _, stats = plan.finalize(want_g3=False)
         if world > 1:
             counts = merge_counts(counts)            # one sum of the 2 MiB histogram per run
-        g = plan.normalize(counts, stats[0] * world)
+        frames_all = stats[0]
+        if world > 1:
+            from paper_1708_08619_b200.sharding import merge_frames
+            frames_all = merge_frames(stats[0], device="cuda")
+        g = plan.normalize(counts, frames_all)
         return counts, g, stats
 
     def step_host():
@@ -269,6 +364,7 @@ def run_ours(args):
     if world > 1:
         dist.all_reduce(tot)
     triplets_all = int(tot.item())
+    frames_all_ranks = F_total if args.shard_one_trajectory else F * world
 
     for _ in range(2):
         step_host()
@@ -287,13 +383,17 @@ def run_ours(args):
     tri_s = tri_ns * 1e-9 / max(tri_launches, 1)                       # avg triplet-kernel launch
     trip_per_launch = triplets_rank * args.steps / max(tri_launches, 1)
     achieved = trip_per_launch * ALGO_INSTR_PER_TRIPLET / tri_s / 1e12 if tri_s > 0 else 0.0
+    batch = plan.info(g3.G3_INFO_BATCH_FRAMES)
+    tri_traffic, tri_traffic_src = ncu_traffic("tiled_triplet_kernel", batch)
+    nb_traffic, _ = ncu_traffic("neighbour_cell_kernel", batch)
+    alg_bytes_per_launch = min(batch, F) * w.n * 24              # N x 24 B of positions per frame
     roofline = {
         "bound": "alu", "kernel": "tiled_triplet_kernel", "achieved": achieved, "peak": peak_tinstr,
         "unit": "Tinstr/s", "frac": achieved / peak_tinstr,
-        "traffic": (NCU_TRIPLET_DRAM_BYTES_PER_LAUNCH
-                    if plan.info(g3.G3_INFO_BATCH_FRAMES) == NCU_TRIPLET_FRAMES_PER_LAUNCH and not args.frames
-                    else None),
-        "traffic_unit": "bytes of DRAM traffic per launch (ncu, profiles/r1_triplet_kernel.md)",
+        "traffic": tri_traffic,
+        "traffic_unit": f"bytes of DRAM traffic per launch (ncu --set full, {tri_traffic_src})",
+        "traffic_algorithmic_bytes": alg_bytes_per_launch,
+        "neighbour_kernel_traffic": nb_traffic,
         "peak_kind": f"{sm_count} SMs x {SM_LANES} lanes x sm_max_mhz ({pk_kind}); DESIGN.md 6",
         "algorithmic_instr_per_triplet": ALGO_INSTR_PER_TRIPLET,
         "triplets_per_launch": trip_per_launch, "kernel_ms_per_launch": tri_s * 1e3,
@@ -302,6 +402,7 @@ def run_ours(args):
         "neighbour_kernel_share_of_step": nb_ns * 1e-6 / args.steps / ms_dev,
         "kernel_triplets_per_s": trip_per_launch / tri_s if tri_s > 0 else 0.0,
         "whole_step_frac": triplets_rank / (ms_dev * 1e-3) * ALGO_INSTR_PER_TRIPLET / 1e12 / peak_tinstr,
+        "neighbour_kernel_ms_per_launch": nb_ns * 1e-6 / max(tri_launches, 1),
         "hbm_gbs_achieved_step": F * w.n * 24 / (ms_dev * 1e-3) / 1e9,
         "hbm_gbs_peak": pk.get("hbm_gbs"),
     }
@@ -332,8 +433,13 @@ def run_ours(args):
             step_q()
             ms_q, (qh, qs), _, _ = timed(step_q, 2)
             extra = max(ms_q - ms_dev, 1e-6)
+            rate = qs[0] / (extra * 1e-3)
             qtet = {"atoms_binned_per_step": qs[0], "extra_ms_per_step": extra,
-                    "atoms_per_s_extra": qs[0] / (extra * 1e-3), "bins": 200}
+                    "atoms_per_s_extra": rate, "bins": 200,
+                    "roofline": {"bound": "alu", "unit": "Tinstr/s", "peak": peak_tinstr,
+                                 "algorithmic_instr_per_atom": ALGO_INSTR_PER_QTET_ATOM,
+                                 "achieved": rate * ALGO_INSTR_PER_QTET_ATOM / 1e12,
+                                 "frac": rate * ALGO_INSTR_PER_QTET_ATOM / 1e12 / peak_tinstr}}
     except Exception as e:  # the g3 numbers above stay valid
         qtet = {"error": str(e)}
     # MSD over all time origins at the same shape (unwrapped random walk,
@@ -351,42 +457,96 @@ def run_ours(args):
         torch.cuda.synchronize()
         ms_msd = e0.elapsed_time(e1) / 3
         disp = w.n * F * (F + 1) // 2
-        msd = {"ms": ms_msd, "displacements_per_s": disp / (ms_msd * 1e-3), "frames": F, "lags": F,
-               "hbm_gbs_achieved": F * w.n * 24 / (ms_msd * 1e-3) / 1e9}
+        rate = disp / (ms_msd * 1e-3)
+        msd = {"ms": ms_msd, "displacements_per_s": rate, "frames": F, "lags": F,
+               "hbm_gbs_achieved": F * w.n * 24 / (ms_msd * 1e-3) / 1e9,
+               "roofline": {"bound": "alu", "unit": "Tinstr/s", "peak": peak_tinstr,
+                            "algorithmic_instr_per_displacement": ALGO_INSTR_PER_DISPLACEMENT,
+                            "achieved": rate * ALGO_INSTR_PER_DISPLACEMENT / 1e12,
+                            "frac": rate * ALGO_INSTR_PER_DISPLACEMENT / 1e12 / peak_tinstr,
+                            "note": "with every lag the kernel is bound by integer issue and shared-memory "
+                                    "loads, not by HBM (algorithmic bytes F x N x 24 are read once)"}}
         del d_walk
     except Exception as e:  # the g3 numbers above stay valid
         msd = {"error": str(e)}
+    others = None
+    if world == 1 and not args.no_other_configs and not args.frames:
+        others = other_configs_leg(g3, torch, stream, peak_tinstr, args.other_steps)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu, _, _, _ = cpu_baseline_leg(w, args.cpu_budget)
+        cpu = cpu_baseline_leg(w, args.cpu_budget)
     nbytes = w.n_r * w.n_r * w.n_t * 8
     line = {
         "metric": METRIC, "value": triplets_all / (ms_dev * 1e-3), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_dev,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+int64",
-        "data": "synthetic", "frames_per_s": F * world / (ms_dev * 1e-3),
+        "higher_is_better": True, "scaling": "strong" if args.shard_one_trajectory else "weak",
+        "vs_baseline": None, "dtype": "f32+int64",
+        "data": "synthetic", "frames_per_s": frames_all_ranks / (ms_dev * 1e-3),
         "config": {"workload": f"config4 {w.name}: N={w.n}, L={w.box}, r_max={w.r_max}, "
-                               f"{w.n_r}x{w.n_r}x{w.n_t} bins, {F} frames per step per GPU",
-                   "frames_per_step": F, "triplets_per_step": triplets_all,
+                               f"{w.n_r}x{w.n_r}x{w.n_t} bins, {frames_all_ranks} frames per step over {world} GPU(s)",
+                   "frames_per_step": frames_all_ranks, "triplets_per_step": triplets_all,
                    "batch_frames": plan.info(g3.G3_INFO_BATCH_FRAMES),
                    "kernel": plan.info(g3.G3_INFO_KERNEL),
                    "l2": f"inputs larger than L2 ({F * w.n * 24 / 2**20:.0f} MiB of positions per step)",
-                   "parallelism": f"frames sharded over {world} GPU(s), one histogram sum per run"},
+                   "parallelism": (f"one trajectory, frames sharded over {world} GPU(s)" if args.shard_one_trajectory
+                                   else f"one trajectory per GPU ({world} GPU(s))") + ", one histogram sum per run"},
         "clocks": clocks,
         "e2e": {"value": triplets_all / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
-                "frames_per_s": F * world / (ms_e2e * 1e-3),
+                "frames_per_s": frames_all_ranks / (ms_e2e * 1e-3),
                 "h2d_bytes_per_step": F * w.n * 24, "d2h_bytes_per_step": 2 * nbytes + 24},
         "gpu_launches": launches * args.steps,
         "gpu_launches_per_step": launches,
         "roofline": roofline,
         "qtet": qtet,
         "msd": msd,
+        "configs": others,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
     plan.close()
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def launch_ranks(args) -> int:
+    """`python bench.py --gpus N` without torchrun: start the N ranks here, one per GPU, through
+    torch.distributed.run on 127.0.0.1 (split the trajectory, merge the
+    results).  NCCL's communicator log is left on so that the ranks can be counted from stderr."""
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    env.setdefault("MASTER_ADDR", "127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd, env=env).returncode
+
+
+def run_launch_check(args) -> int:
+    """What the launcher starts, without a GPU: every rank joins a gloo group, reports its rank
+    and the block of frames --shard-one-trajectory would give it; rank 0 prints one JSON line."""
+    import torch
+    import torch.distributed as dist
+    from paper_1708_08619_b200.sharding import frame_shard
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    F = args.frames or WORKLOADS[WORKLOAD_INDEX].n_frames
+    b, e = frame_shard(F, rank, world)
+    mine = torch.tensor([rank, b, e, os.getpid()], dtype=torch.int64)
+    rows = [mine]
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("gloo")
+        rows = [torch.zeros(4, dtype=torch.int64) for _ in range(world)]
+        dist.all_gather(rows, mine)
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"launched": world, "ranks": [int(r[0]) for r in rows],
+                          "shards": [[int(r[1]), int(r[2])] for r in rows],
+                          "pids": [int(r[3]) for r in rows], "frames": F}), flush=True)
     return 0
 
 
@@ -402,7 +562,17 @@ def main():
     ap.add_argument("--ref-frames", type=int, default=4, help="frames per step of --impl reference")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the configs 1, 2, 3, 5 block")
+    ap.add_argument("--other-steps", type=int, default=2)
+    ap.add_argument("--shard-one-trajectory", action="store_true",
+                    help="strong scaling: split the one seeded trajectory over the ranks (sharding.frame_shard)")
+    ap.add_argument("--launch-check", action="store_true",
+                    help="CPU only: start the ranks (gloo), report rank count and frame shards, no GPU work")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return launch_ranks(args)
+    if args.launch_check:
+        return run_launch_check(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -118,6 +118,9 @@ int configure(g3_plan* p) {
         p->batch_frames = (int32_t)std::min<int64_t>(std::max<int64_t>(want, 16), 256);
     }
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled
+    // q_tet straight from the shell-sorted neighbour lists of the tiled path (qtet_list_kernel);
+    // plans served by the generic kernel have no lists and use the 27-cell scan of g3_qtet.cuh
+    p->qtet_lists = p->qtet_bins > 0 && p->kernel == 2 && (int64_t)p->batch_frames * p->n < (int64_t(1) << 31);
     if (p->kernel == 1) {
         size_t smem = generic_smem_bytes(p->bins.n_r, p->bins.n_t, p->max_nb, kGenericWarps);
         if (smem > (size_t)p->smem_optin) return G3_EINVAL;   // neighbour capacity too large
@@ -142,7 +145,10 @@ int configure(g3_plan* p) {
         G3_CUDA(cudaMemset(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2));
         G3_CUDA(allow_max_dynamic_smem(qtet_kernel<kQtetWarps>, p->smem_optin));
         G3_CUDA(allow_max_dynamic_smem(qtet_redo_kernel<kQtetWarps>, p->smem_optin));
-        if (p->ncell > 1 && B * n < (int64_t(1) << 31)) {   // fast path: 27 cells staged per CTA
+        G3_CUDA(allow_max_dynamic_smem(qtet_list_kernel, p->smem_optin));
+        if (p->qtet_lists) {                                // only the list of undecided atoms is needed
+            G3_CUDA(cudaMalloc(&p->d_qtet_redo, sizeof(int32_t) * (size_t)(B * n + 1)));
+        } else if (p->ncell > 1 && B * n < (int64_t(1) << 31)) {   // fast path: 27 cells staged per CTA
             p->qtet_stage_cap = tiled_stage_cap(p);
             const size_t smem = qtet_cell_smem_bytes(p->qtet_stage_cap, p->qtet_bins);
             if (smem <= (size_t)p->smem_optin) {
@@ -197,7 +203,17 @@ int flush(g3_plan* p, cudaStream_t st) {
         QtParams qp{p->qtet_bins, (double)p->qtet_bins / 4.0, cw * cw, p->d_qtet, p->d_qtet_stats,
                     p->qtet_stage_cap, p->d_qtet_origin, p->d_qtet_redo, 0};
         const size_t hist_smem = sizeof(unsigned int) * p->qtet_bins;
-        if (p->d_qtet_redo) {
+        if (p->qtet_lists) {
+            // the four nearest neighbours sit at the head of the shell-sorted lists this batch's
+            // neighbour kernel has just written; atoms with fewer than four go to the exact routine
+            G3_CUDA(cudaMemsetAsync(p->d_qtet_redo, 0, sizeof(int32_t), st));
+            const g3::TiledState* ts = p->tiled;
+            qtet_list_kernel<<<(unsigned)std::min<long long>((total + 255) / 256, (long long)p->sm_count * 8), 256,
+                               hist_smem, st>>>(ts->d_nbv, ts->d_nbj, ts->d_nbcount, total, p->max_nb, qp);
+            qp.use_redo = 1;
+            qtet_redo_kernel<kQtetWarps><<<(unsigned)p->sm_count * 2, kQtetWarps * 32, hist_smem, st>>>(fb, qp);
+            p->launches += 2;
+        } else if (p->d_qtet_redo) {
             G3_CUDA(cudaMemsetAsync(p->d_qtet_redo, 0, sizeof(int32_t), st));
             const long long items = (long long)nc3 * F;
             // persistent: exactly the CTAs that are resident together (a larger grid would run a second wave)

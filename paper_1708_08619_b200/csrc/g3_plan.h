@@ -89,6 +89,7 @@ struct g3_plan {
     int32_t* d_qtet_redo = nullptr;          // [1 + batch * n]: atoms handed to the exact routine
     int4* d_qtet_origin = nullptr;           // [ncell3] cell centres on the grid
     int32_t qtet_stage_cap = 0;
+    bool qtet_lists = false;                 // q_tet taken from the shell-sorted neighbour lists (qtet_list_kernel)
     int4* d_staged = nullptr;                // [batch][n] quantised (x,y,z,cell) in input order
     int32_t* d_slot = nullptr;               // [batch][n] rank of the particle inside its cell
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]

@@ -26,28 +26,9 @@
 #include "g3_generic.cuh"
 #include "g3_neighbour.cuh"
 #include "g3_plan.h"
+#include "g3_qtet_eq.cuh"
 
 namespace g3 {
-
-struct QtParams {
-    int32_t n_q;                          // bins on [-3, 1]
-    double scale;                         // n_q / 4
-    unsigned long long guarantee2;        // (cell width)^2: below it the 27-cell search is exact
-    unsigned long long* hist;             // [n_q]
-    unsigned long long* stats;            // [2]: atoms binned, atoms skipped
-    int32_t stage_cap;                    // qtet_cell_kernel: staged candidates per CTA
-    const int4* cell_origin;              // [ncell3] grid coordinates of the cell centres
-    int32_t* redo;                        // [frames * n + 1]: count, then atoms handed to qtet_kernel
-    int32_t use_redo;                     // qtet_kernel: 1 = process the redo list, 0 = every atom
-};
-
-struct QtKey {
-    unsigned long long hi, lo;            // d2; (dx, dy, dz) + 2^19 packed 20 bits each
-};
-
-__device__ __forceinline__ bool qt_lt(const QtKey& a, const QtKey& b) {
-    return a.hi < b.hi || (a.hi == b.hi && a.lo < b.lo);
-}
 
 __device__ __forceinline__ void qt_insert(QtKey (&top)[4], const QtKey k) {
     if (!qt_lt(k, top[3])) return;
@@ -92,38 +73,6 @@ __device__ __forceinline__ void qt_merge(QtKey (&top)[4], int lane, QtKey (&best
             top[3].hi = ~0ull; top[3].lo = ~0ull;
         }
     }
-}
-
-// Eq. 1 for one atom from its four nearest neighbours `best` (sorted by key), evaluated by one
-// lane in fp64, one rounding per operation, in the order of reading T2; then the bin (T3, T4).
-__device__ __forceinline__ void qt_finish(const QtKey (&best)[4], const QtParams& qp, unsigned int* hist_s,
-                                          unsigned long long& binned, unsigned long long& skipped) {
-    if (best[3].hi == ~0ull || best[0].hi == 0ull) { skipped += 1; return; }       // T4
-    double nrm[4];
-    long long vx[4], vy[4], vz[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        nrm[j] = __dsqrt_rn((double)best[j].hi);
-        vx[j] = (long long)(best[j].lo >> 40) - 524288;
-        vy[j] = (long long)((best[j].lo >> 20) & 0xFFFFF) - 524288;
-        vz[j] = (long long)(best[j].lo & 0xFFFFF) - 524288;
-    }
-    double acc = 0.0;
-#pragma unroll
-    for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int k = j + 1; k < 4; ++k) {
-            const long long dot = vx[j] * vx[k] + vy[j] * vy[k] + vz[j] * vz[k];
-            const double den = __dmul_rn(nrm[j], nrm[k]);
-            const double c = __ddiv_rn((double)dot, den);
-            const double t = __dadd_rn(c, 1.0 / 3.0);
-            acc = __dadd_rn(acc, __dmul_rn(t, t));
-        }
-    const double q = __dsub_rn(1.0, __dmul_rn(0.375, acc));
-    long long b = (long long)floor(__dmul_rn(__dadd_rn(q, 3.0), qp.scale));
-    b = b < 0 ? 0 : (b > qp.n_q - 1 ? qp.n_q - 1 : b);
-    atomicAdd(hist_s + b, 1u);
-    binned += 1;
 }
 
 __device__ __forceinline__ void qt_flush(const QtParams& qp, const unsigned int* hist_s,
@@ -219,6 +168,48 @@ qtet_redo_kernel(FrameBatch fb, QtParams qp) {
             qt_merge(top, lane, best);
             if (lane == 0) qt_finish(best, qp, qt_hist, binned, skipped);
         }
+    }
+    qt_flush(qp, qt_hist, binned, skipped);
+}
+
+// q_tet from the neighbour lists of the tiled g(3) path (g3_neighbour.cuh): nbv[atom][e] =
+// (dx, dy, dz, .) exact minimum-image vectors of ALL particles inside r_max, sorted by shell of
+// r_ij; nbj[atom][e] grows strictly with the shell.  With k >= 4 entries the four nearest
+// neighbours are among the entries whose shell is not beyond the shell of the fourth entry (every
+// entry of a lower shell is nearer than every entry of a higher one, and every particle outside
+// the list is farther than all of them).  One THREAD per atom: exact keys of those few entries,
+// top four by insertion, Eq. 1 in fp64 (reading T2).  Atoms with k < 4 go to qtet_redo_kernel.
+__global__ void __launch_bounds__(256)
+qtet_list_kernel(const float4* __restrict__ nbv, const uint32_t* __restrict__ nbj, const int32_t* __restrict__ nbcount,
+                 long long total, int32_t max_nb, QtParams qp) {
+    extern __shared__ unsigned int qt_hist[];
+    for (int32_t i = threadIdx.x; i < qp.n_q; i += blockDim.x) qt_hist[i] = 0;
+    __syncthreads();
+    unsigned long long binned = 0, skipped = 0;
+    for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long long)gridDim.x * blockDim.x) {
+        const int32_t k = nbcount[g];
+        if (k < 4) {                                       // the fourth neighbour is beyond r_max: all particles
+            const int32_t idx = atomicAdd(qp.redo, 1);
+            qp.redo[1 + idx] = (int32_t)g;
+            continue;
+        }
+        const float4* __restrict__ lv = nbv + g * max_nb;
+        const uint32_t* __restrict__ lj = nbj + g * max_nb;
+        const uint32_t shell4 = lj[3];
+        QtKey top[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) { top[t].hi = ~0ull; top[t].lo = ~0ull; }
+        for (int32_t e = 0; e < k; ++e) {
+            if (e >= 4 && lj[e] > shell4) break;           // sorted by shell: nothing nearer follows
+            const float4 v = lv[e];
+            const long long X = (long long)v.x, Y = (long long)v.y, Z = (long long)v.z;
+            QtKey key;
+            key.hi = (unsigned long long)(X * X + Y * Y + Z * Z);
+            key.lo = ((unsigned long long)(X + 524288) << 40) | ((unsigned long long)(Y + 524288) << 20) |
+                     (unsigned long long)(Z + 524288);
+            qt_insert(top, key);
+        }
+        qt_finish(top, qp, qt_hist, binned, skipped);
     }
     qt_flush(qp, qt_hist, binned, skipped);
 }

@@ -95,3 +95,22 @@ def test_merge_without_process_group_is_identity():
     y = merge_counts(x)
     assert y.equal(x) and y.data_ptr() != x.data_ptr()
     assert merge_frames(7) == 7
+
+
+def test_bench_launches_its_own_ranks():
+    """`python bench.py --gpus N` (no torchrun, WORLD_SIZE unset) must start N ranks itself
+    (PAPER.md:356, 727).  --launch-check runs them on CPU over gloo: every rank reports its rank,
+    pid and the frame block --shard-one-trajectory would give it."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "3", "--launch-check",
+                          "--frames", "500"], env=env, capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["launched"] == 3 and line["ranks"] == [0, 1, 2]
+    assert len(set(line["pids"])) == 3
+    assert line["shards"] == [list(frame_shard(500, r, 3)) for r in range(3)]
+    assert line["shards"][0][0] == 0 and line["shards"][-1][1] == 500
