@@ -595,7 +595,8 @@ int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_strid
     G3_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
     if (cc_major < 10) return G3_ECUDA;
     const int32_t n_blocks = (int32_t)((n + kMsdAtoms - 1) / kMsdAtoms);
-    const size_t traj_smem = (size_t)n_frames * kMsdAtoms * 3 * sizeof(int32_t);
+    // trajectories of 32 atoms + the prefix table of their squares
+    const size_t traj_smem = (size_t)n_frames * kMsdAtoms * 3 * sizeof(int32_t) + (size_t)(n_frames + 1) * sizeof(ulonglong2);
     const bool smem_path = traj_smem <= (size_t)smem_optin;
     MsdParams mp;
     mp.pos = d_pos; mp.stride = frame_stride; mp.n = (int32_t)n; mp.n_frames = (int32_t)n_frames;
@@ -610,13 +611,12 @@ int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_strid
     auto fail = [&](int code) { cudaFreeAsync(ws, st); cudaGetLastError(); return code; };
     if (cudaMemsetAsync(mp.bad, 0, 16, st) != cudaSuccess) return fail(G3_ECUDA);
     if (smem_path) {
-        if (cudaFuncSetAttribute(msd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)traj_smem) != cudaSuccess) return fail(G3_ECUDA);
-        msd_kernel<true><<<n_blocks, kMsdWarps * 32, traj_smem, st>>>(mp);
+        if (allow_max_dynamic_smem(msd_kernel, smem_optin) != cudaSuccess) return fail(G3_ECUDA);
+        msd_kernel<<<n_blocks, kMsdWarps * 32, traj_smem, st>>>(mp);
     } else {
         mp.snapped = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + part_bytes + 16);
         msd_snap_kernel<<<sm_count * 8, 256, 0, st>>>(mp);
-        msd_kernel<false><<<n_blocks, kMsdWarps * 32, 0, st>>>(mp);
+        msd_direct_kernel<<<n_blocks, kMsdWarps * 32, 0, st>>>(mp);
     }
     const double g = box / 1048576.0;
     msd_reduce_kernel<<<(unsigned)((max_lag + 128) / 128), 128, 0, st>>>(

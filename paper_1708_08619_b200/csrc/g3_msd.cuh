@@ -6,11 +6,13 @@
 // (F - dt) origins per lag balance out).  The unwrapped positions are snapped to the box/2^20 grid
 // once (m = llrint(x 2^20 / box), no wrap: DESIGN.md reading M1) and every squared displacement
 // is an exact integer, accumulated in 128 bits (M2).
-//   msd_kernel<true>   the 32 trajectories of the CTA are staged in shared memory as int32
-//                      [F][32][3] (lane stride 3 words: conflict-free), so HBM is read once:
-//                      F x 384 B must fit shared memory (F <= ~590);
-//   msd_kernel<false>  longer trajectories: the same loops over a snapped int32 copy in global
-//                      memory ([F][n][3], written by msd_snap_kernel).
+//   msd_kernel          the 32 trajectories of the CTA are staged in shared memory as int32
+//                       [F][32][3] (lane stride 3 words: conflict-free), so HBM is read once:
+//                       F x 400 B must fit shared memory (F <= ~580); squares through a prefix
+//                       table, cross terms with four adjacent lags per warp (see the kernel);
+//   msd_direct_kernel   longer trajectories: the direct loops (four strided lags per warp share
+//                       the origin loads) over a snapped int32 copy in global memory ([F][n][3],
+//                       written by msd_snap_kernel).
 // A warp sums its 32 atoms with shuffles and writes one 128-bit partial per (CTA, lag);
 // msd_reduce_kernel adds the partials of a lag and evaluates msd[dt] in fp64 (M3).
 #pragma once
@@ -52,28 +54,186 @@ msd_snap_kernel(MsdParams mp) {
     if (bad) atomicAdd(mp.bad, bad);
 }
 
-template <bool kSmem>
+// 128-bit helpers on (lo, hi) pairs, arithmetic mod 2^128
+__device__ __forceinline__ void u128_add(unsigned long long& lo, unsigned long long& hi, unsigned long long alo,
+                                         unsigned long long ahi) {
+    lo += alo;
+    hi += ahi + (lo < alo ? 1ull : 0ull);
+}
+
+__device__ __forceinline__ void u128_sub(unsigned long long& lo, unsigned long long& hi, unsigned long long alo,
+                                         unsigned long long ahi) {
+    const unsigned long long borrow = lo < alo ? 1ull : 0ull;
+    lo -= alo;
+    hi -= ahi + borrow;
+}
+
+// add the sign-extended 64-bit value s
+__device__ __forceinline__ void u128_add_s64(unsigned long long& lo, unsigned long long& hi, long long s) {
+    u128_add(lo, hi, (unsigned long long)s, (unsigned long long)(s >> 63));
+}
+
+// msd_kernel: trajectories of 32 atoms staged in shared memory (F x 384 B + the prefix table).
+//   sum_t |r(t+dt) - r(t)|^2 = sum_t |r(t+dt)|^2 + sum_t |r(t)|^2 - 2 sum_t r(t+dt).r(t)
+// The first two sums are differences of ONE prefix table P[t] = sum_{u<t} sum_atoms |r(u)|^2 per
+// CTA (O(F) work); only the cross term needs all (origin, lag) pairs: three multiply-adds per
+// displacement.  |m| < 2^30, so a dot product is below 3 * 2^60 and two of them fit a signed
+// 64-bit word before they are folded into a 128-bit sum; every quantity is an exact integer and
+// the result is the same 128-bit sum as the direct evaluation (reading M2).
+// A warp takes FOUR ADJACENT lags: moving the origin by one frame shifts their windows by one
+// frame, so each step loads one new origin and one new end point (6 LDS for 4 displacements).
 __global__ void __launch_bounds__(kMsdWarps * 32)
 msd_kernel(MsdParams mp) {
-    extern __shared__ int32_t msd_traj[];                  // [F][32][3] (kSmem)
+    extern __shared__ __align__(16) int32_t msd_traj[];    // [F][32][3], then ulonglong2 P[F + 1]
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int32_t atom = blockIdx.x * kMsdAtoms + lane;
     const bool valid = atom < mp.n;
     const int32_t F = mp.n_frames;
-    if (kSmem) {
+    ulonglong2* P = reinterpret_cast<ulonglong2*>(msd_traj + (size_t)F * kMsdAtoms * 3);
+    __shared__ unsigned int range_s;                      // OR of |m| over the CTA's coordinates
+    if (threadIdx.x == 0) range_s = 0;
+    __syncthreads();
+    {
         unsigned long long bad = 0;
+        unsigned int range = 0;
         for (int32_t t = wid; t < F; t += kMsdWarps) {
             const double* row = mp.pos + (long long)t * mp.stride + 3ll * atom;
+            int32_t m[3];
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
-                msd_traj[(t * kMsdAtoms + lane) * 3 + c] = valid ? msd_snap(row[c], mp.inv_g, bad) : 0;
+            for (int c = 0; c < 3; ++c) {
+                m[c] = valid ? msd_snap(row[c], mp.inv_g, bad) : 0;
+                msd_traj[(t * kMsdAtoms + lane) * 3 + c] = m[c];
+                range |= (unsigned int)abs(m[c]);
+            }
+            // sum over the CTA's atoms of |r(t)|^2 (< 32 * 3 * 2^60): 32-bit halves summed in 64 bits
+            const unsigned long long q = (unsigned long long)((long long)m[0] * m[0]) + (unsigned long long)((long long)m[1] * m[1]) +
+                                         (unsigned long long)((long long)m[2] * m[2]);
+            unsigned long long ql = q & 0xFFFFFFFFull, qh = q >> 32;
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                ql += __shfl_xor_sync(0xffffffffu, ql, d);
+                qh += __shfl_xor_sync(0xffffffffu, qh, d);
+            }
+            if (lane == 0) {
+                unsigned long long lo = ql, hi = 0;
+                u128_add(lo, hi, qh << 32, qh >> 32);
+                P[t + 1] = make_ulonglong2(lo, hi);
+            }
         }
         if (bad) atomicAdd(mp.bad, bad);
-        __syncthreads();
+        range = __reduce_or_sync(0xffffffffu, range);
+        if (lane == 0) atomicOr(&range_s, range);
     }
-    // element (t, this atom, c): shared [t][lane][c] or global [t][atom][c]
-    const int32_t* base = kSmem ? msd_traj + lane * 3 : mp.snapped + 3ll * (valid ? atom : 0);
-    const long long tstride = kSmem ? kMsdAtoms * 3 : 3ll * mp.n;
+    __syncthreads();
+    // |m| < 2^28 for every coordinate of this CTA: a dot product is below 3 * 2^56 and 32 of them
+    // fit a signed 64-bit word, so the 128-bit fold runs once per 32 origins instead of once per 2
+    const bool narrow = range_s < (1u << 28);
+    if (threadIdx.x == 0) {                               // exclusive prefix over the frames
+        unsigned long long lo = 0, hi = 0;
+        P[0] = make_ulonglong2(0ull, 0ull);
+        for (int32_t t = 1; t <= F; ++t) {
+            const ulonglong2 v = P[t];
+            u128_add(lo, hi, v.x, v.y);
+            P[t] = make_ulonglong2(lo, hi);
+        }
+    }
+    __syncthreads();
+
+    const int32_t* base = msd_traj + lane * 3;             // element (t, this atom, c) = base[t * 96 + c]
+    constexpr int32_t TS = kMsdAtoms * 3;
+    const int32_t n_groups = (mp.max_lag + 4) >> 2;        // groups of four adjacent lags
+    for (int32_t grp = wid; grp < n_groups; grp += kMsdWarps) {
+        const int32_t d0 = grp << 2;
+        unsigned long long lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};
+        const int32_t n_full = F - d0 - 3;                 // origins for which all four lags exist
+        int32_t t = 0;
+        if (n_full >= 4) {
+            int32_t bx[4], by[4], bz[4];                   // b[x & 3] = r(t + d0 + x) for the four lags of a step
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const int32_t* b = base + (d0 + x) * TS;
+                bx[x] = b[0]; by[x] = b[1]; bz[x] = b[2];
+            }
+            long long acc[4] = {0, 0, 0, 0};
+            const int32_t* a = base;
+            const int32_t* e = base + (d0 + 3) * TS;
+#define G3_MSD_STEP(i)                                                                             \
+            {                                                                                      \
+                const int32_t ax = a[(i) * TS], ay = a[(i) * TS + 1], az = a[(i) * TS + 2];        \
+                bx[((i) + 3) & 3] = e[(i) * TS]; by[((i) + 3) & 3] = e[(i) * TS + 1]; bz[((i) + 3) & 3] = e[(i) * TS + 2]; \
+                _Pragma("unroll")                                                                  \
+                for (int jj = 0; jj < 4; ++jj)                                                     \
+                    acc[jj] += (long long)ax * bx[((i) + jj) & 3] + (long long)ay * by[((i) + jj) & 3] + \
+                               (long long)az * bz[((i) + jj) & 3];                                 \
+            }
+#define G3_MSD_FOLD()                                                                              \
+            _Pragma("unroll")                                                                      \
+            for (int jj = 0; jj < 4; ++jj) { u128_add_s64(lo[jj], hi[jj], acc[jj]); acc[jj] = 0; }
+            if (narrow) {
+                for (; t + 32 <= n_full; t += 32) {
+#pragma unroll 1
+                    for (int u = 0; u < 8; ++u) {
+                        G3_MSD_STEP(0) G3_MSD_STEP(1) G3_MSD_STEP(2) G3_MSD_STEP(3)
+                        a += 4 * TS; e += 4 * TS;
+                    }
+                    G3_MSD_FOLD()
+                }
+            }
+            for (; t + 4 <= n_full; t += 4) {
+                G3_MSD_STEP(0) G3_MSD_STEP(1) G3_MSD_FOLD()
+                G3_MSD_STEP(2) G3_MSD_STEP(3) G3_MSD_FOLD()
+                a += 4 * TS; e += 4 * TS;
+            }
+#undef G3_MSD_STEP
+#undef G3_MSD_FOLD
+        }
+        // the remaining origins (fewer than four, plus those that exist only for the shorter lags)
+        for (; t < F - d0; ++t) {
+            const int32_t* a = base + t * TS;
+            const int32_t ax = a[0], ay = a[1], az = a[2];
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                if (t + d0 + jj < F) {
+                    const int32_t* b = a + (d0 + jj) * TS;
+                    u128_add_s64(lo[jj], hi[jj], (long long)ax * b[0] + (long long)ay * b[1] + (long long)az * b[2]);
+                }
+            }
+        }
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const int32_t dt = d0 + jj;
+            if (dt > mp.max_lag) break;                    // uniform over the warp
+            unsigned long long l = lo[jj], h = hi[jj];     // cross term of this lane's atom
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                const unsigned long long olo = __shfl_xor_sync(0xffffffffu, l, d);
+                const unsigned long long ohi = __shfl_xor_sync(0xffffffffu, h, d);
+                l += olo;
+                h += ohi + (l < olo ? 1ull : 0ull);
+            }
+            if (lane == 0) {
+                // S = P[F - dt] + (P[F] - P[dt]) - 2 C
+                const ulonglong2 p1 = P[F - dt], p2 = P[F], p3 = P[dt];
+                unsigned long long slo = p1.x, shi = p1.y;
+                u128_add(slo, shi, p2.x, p2.y);
+                u128_sub(slo, shi, p3.x, p3.y);
+                u128_sub(slo, shi, l, h);
+                u128_sub(slo, shi, l, h);
+                mp.partial[(size_t)blockIdx.x * (mp.max_lag + 1) + dt] = make_ulonglong2(slo, shi);
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kMsdWarps * 32)
+msd_direct_kernel(MsdParams mp) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t atom = blockIdx.x * kMsdAtoms + lane;
+    const bool valid = atom < mp.n;
+    const int32_t F = mp.n_frames;
+    // element (t, this atom, c) of the snapped copy: global [t][atom][c]
+    const int32_t* base = mp.snapped + 3ll * (valid ? atom : 0);
+    const long long tstride = 3ll * mp.n;
     // Four lags per pass share the loads of the origin r(t): lags dt, dt + W, dt + 2W, dt + 3W.
     // |m| < 2^30, so a displacement component fits int32 and its square is one 32 x 32 -> 64 multiply.
     auto sq = [](int32_t dx, int32_t dy, int32_t dz) {
