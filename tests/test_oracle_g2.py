@@ -42,6 +42,52 @@ def test_lattice_worked_example(oracle_lib):
     assert np.array_equal(H2, want)
 
 
+def wide_thresholds(oracle_lib, box, r_max, n_r):
+    """squared shell edges b w, b = 0..2 n_r, with the neighbour shells' own width w = r_max / n_r:
+    (2 r_max) / (2 n_r) is the same double as r_max / n_r, so the first n_r + 1 edges are T_r itself"""
+    T2, _ = oracle_lib.thresholds(box, 2.0 * r_max, 2 * n_r, 1)
+    T_r, _ = oracle_lib.thresholds(box, r_max, n_r, 1)
+    assert np.array_equal(T2[: n_r + 1], T_r)
+    return T2
+
+
+def test_hand_derived_lattice_over_the_whole_rjk_range(oracle_lib):
+    """tests/golden/lattice_8x8x8_g2_wide.txt: g2 counted to 2 r_max (the r_jk axis of g3)"""
+    g = np.arange(8, dtype=np.int32) << 17
+    m = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3)
+    T2 = wide_thresholds(oracle_lib, 8.0, 1.05, 7)
+    H2 = oracle_lib.g2_frame(m, T2)
+    want = np.zeros(14, dtype=np.uint64)
+    with open(os.path.join(GOLDEN, "lattice_8x8x8_g2_wide.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                a, c = line.split()
+                want[int(a)] = int(c)
+    assert want.sum() == 512 * 32
+    assert np.array_equal(H2, want)
+    # the lower half is the neighbour-range histogram
+    T_r, _ = oracle_lib.thresholds(8.0, 1.05, 7, 1)
+    assert np.array_equal(oracle_lib.g2_frame(m, T_r), want[:7])
+
+
+def test_wide_range_against_numpy_and_ideal_gas(oracle_lib):
+    """numpy all-pairs count over [0, 2 r_max) and the ideal-gas value (N-1)/N in every shell"""
+    w = WORKLOADS[2]
+    m, _ = frames(w, 1)
+    m = m[0][:700]
+    T2 = wide_thresholds(oracle_lib, w.box, w.r_max, w.n_r)
+    ref, _ = numpy_pair_counts(m, T2)
+    assert np.array_equal(oracle_lib.g2_frame(m, T2), ref)
+    n, box, r_max, n_r = 3000, 10.0, 1.2, 6                  # 2 r_max = 2.4 < box / 2
+    H2 = np.zeros(2 * n_r, dtype=np.uint64)
+    T2 = wide_thresholds(oracle_lib, box, r_max, n_r)
+    for f in range(4):
+        oracle_lib.g2_frame(uniform_frame(n, seed=900 + f), T2, H2)
+    g2 = oracle_lib.g2_normalise(H2, 2.0 * r_max, 4, n, box)
+    z = (g2 / (1.0 - 1.0 / n) - 1.0) * np.sqrt(H2.astype(np.float64) / 2.0)
+    assert np.abs(z[1:]).max() < 5.0
+
+
 def test_against_numpy_definition_and_g3_pair_statistics(oracle_lib):
     for widx, n_take in ((1, 216), (2, 600)):
         w = WORKLOADS[widx]
