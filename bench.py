@@ -442,6 +442,26 @@ def run_ours(args):
                                  "frac": rate * ALGO_INSTR_PER_QTET_ATOM / 1e12 / peak_tinstr}}
     except Exception as e:  # the g3 numbers above stay valid
         qtet = {"error": str(e)}
+    # g2 over the whole r_jk range [0, 2 r_max) (G3_OPT_G2_WIDE), timed as the
+    # EXTRA cost of its second pair search over the g3 path
+    g2w = None
+    try:
+        if world > 1:
+            raise RuntimeError("measured at --gpus 1 only")
+        with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, g2_wide=True) as gplan:
+            def step_g():
+                gplan.reset()
+                gplan.accumulate_frames(d_pos)
+                gplan.finalize(want_g3=False)
+                return gplan.finalize_g2()
+            step_g()
+            ms_g, (c2w, _), _, _ = timed(step_g, 2)
+            extra = max(ms_g - ms_dev, 1e-6)
+            pairs = int(c2w.cpu().numpy().view(np.uint64)[w.n_r:].sum())
+            g2w = {"shells": 2 * w.n_r, "extra_ms_per_step": extra, "outer_ordered_pairs_per_step": pairs,
+                   "outer_pairs_per_s_extra": pairs / (extra * 1e-3)}
+    except Exception as e:  # the g3 numbers above stay valid
+        g2w = {"error": str(e)}
     # MSD over all time origins at the same shape (unwrapped random walk,
     # N = 32768, F frames, every lag), device-resident; CUDA events around the g3_msd calls
     msd = None
@@ -498,6 +518,7 @@ def run_ours(args):
         "gpu_launches_per_step": launches,
         "roofline": roofline,
         "qtet": qtet,
+        "g2_wide": g2w,
         "msd": msd,
         "configs": others,
         "cpu_baseline": cpu,

@@ -84,6 +84,9 @@ typedef enum {
     G3_OPT_QTET_BINS = 6,    /* > 0: also histogram the tetrahedral order parameter q_tet (Eq. 1,
                                 PAPER.md:201) of every atom into this many bins on [-3, 1] while
                                 frames are accumulated; 0 (default) = off; needs n >= 5      */
+    G3_OPT_G2_WIDE = 7,      /* 1 = the pair histogram g2 also covers [r_max, 2 r_max), the rest of the
+                                r_jk axis of g(3), in n_r more shells of the same width (a second
+                                pair search per frame); 0 (default) = the neighbour range only */
     G3_OPT_TIMING = 4         /* 1 = bracket the neighbour and triplet kernels with CUDA events
                                  on the caller's stream (read back with g3_plan_get_info)     */
 } g3_option;
@@ -104,9 +107,10 @@ typedef enum {
     G3_INFO_NEIGHBOUR_NS = 10,   /* device time of the neighbour kernel launches             */
     G3_INFO_TIMED_LAUNCHES = 11, /* launches of EACH of the two kernels covered by the sums
                                     (a triplet "launch" = all slab passes of one batch)      */
-    G3_INFO_SLABS = 12           /* tiled kernel: slab passes per batch (1 = the reachable bins
+    G3_INFO_SLABS = 12,          /* tiled kernel: slab passes per batch (1 = the reachable bins
                                     fit one shared-memory tile; G3_INFO_TILE_BINS counts all
                                     reachable slots, over all slabs)                          */
+    G3_INFO_G2_SHELLS = 13       /* shells g3_finalize_g2 writes: n_r, or 2 n_r with G3_OPT_G2_WIDE */
 } g3_info;
 
 /* Create a plan for frames of `n` particles in a cubic periodic box of edge `box`
@@ -165,14 +169,17 @@ G3_API int g3_finalize(g3_plan *p, uint64_t *d_counts, double *d_g3, uint64_t *h
 /* Same with HOST output buffers (device-to-host copies included).                   */
 G3_API int g3_finalize_host(g3_plan *p, uint64_t *h_counts, double *h_g3, uint64_t *h_stats, void *stream);
 
-/* g2, the pair distribution function, from the same neighbour pass (Algorithm 6 "g2
- * histogram"; Algorithm 7 CUDA_g2; reading G1:
- * the range is the neighbour range [0, r_max) with the n_r shells of r_ij, not the paper's
- * L/2).  Reduces all staged frames like g3_finalize, then, asynchronously on `stream`:
- *   d_counts2  device, uint64 [n_r]: ordered pairs (i, j), j != i, per shell; may be NULL
- *   d_g2       device, fp64 [n_r]: counts2 / (frames n rho V_a), V_a = 4 pi/3 (r_{a+1}^3 - r_a^3),
+/* g2, the pair distribution function (Algorithm 6 "g2 histogram"; Algorithm 7
+ * CUDA_g2; reading G1).  By default over the neighbour range
+ * [0, r_max) with the n_r shells of r_ij, counted in the same neighbour pass; with
+ * G3_OPT_G2_WIDE over [0, 2 r_max), the whole r_jk axis of g(3) (the Kirkwood denominator
+ * g2 g2 g2), in S = 2 n_r shells of the same width (S = G3_INFO_G2_SHELLS).  Minimum-image
+ * distances: shells beyond box/2 (possible only when r_max > box/4) are geometrically incomplete.
+ * Reduces all staged frames like g3_finalize, then, asynchronously on `stream`:
+ *   d_counts2  device, uint64 [S]: ordered pairs (i, j), j != i, per shell; may be NULL
+ *   d_g2       device, fp64 [S]: counts2 / (frames n rho V_a), V_a = 4 pi/3 (r_{a+1}^3 - r_a^3),
  *              rho = n / box^3 (ideal gas -> (n-1)/n); may be NULL
- * Does not synchronise and does not reset.  sum(counts2) = sum_i k_i.                */
+ * Does not synchronise and does not reset.  sum(counts2[0 .. n_r)) = sum_i k_i.       */
 G3_API int g3_finalize_g2(g3_plan *p, uint64_t *d_counts2, double *d_g2, void *stream);
 
 /* q_tet, the tetrahedral order parameter (Eq. 1; Algorithms 2-3),

@@ -16,9 +16,10 @@ LIB_PATH = os.path.join(_HERE, "libg3.so")
 G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
 G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING, G3_OPT_TRIPLET_WARPS = 1, 2, 3, 4, 5
 G3_OPT_QTET_BINS = 6
+G3_OPT_G2_WIDE = 7
 (G3_INFO_KERNEL_LAUNCHES, G3_INFO_BATCH_FRAMES, G3_INFO_KERNEL, G3_INFO_CELLS_PER_EDGE,
  G3_INFO_MAX_NEIGHBOURS, G3_INFO_TILE_BINS, G3_INFO_SM_COUNT, G3_INFO_FRAMES_PENDING,
- G3_INFO_TRIPLET_NS, G3_INFO_NEIGHBOUR_NS, G3_INFO_TIMED_LAUNCHES, G3_INFO_SLABS) = range(1, 13)
+ G3_INFO_TRIPLET_NS, G3_INFO_NEIGHBOUR_NS, G3_INFO_TIMED_LAUNCHES, G3_INFO_SLABS, G3_INFO_G2_SHELLS) = range(1, 14)
 
 EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
@@ -142,7 +143,7 @@ class Plan:
     def __init__(self, n: int, box: float, r_max: float, n_r: int, n_t: Optional[int] = None, *,
                  batch_frames: Optional[int] = None, kernel: Optional[int] = None,
                  max_neighbours: Optional[int] = None, timing: bool = False,
-                 triplet_warps: Optional[int] = None, qtet_bins: Optional[int] = None):
+                 triplet_warps: Optional[int] = None, qtet_bins: Optional[int] = None, g2_wide: bool = False):
         self._lib = load()
         self.n, self.box, self.r_max = int(n), float(box), float(r_max)
         self.n_r, self.n_t = int(n_r), int(n_r if n_t is None else n_t)
@@ -159,6 +160,9 @@ class Plan:
             self.set_option(G3_OPT_TIMING, 1)
         if triplet_warps is not None:
             self.set_option(G3_OPT_TRIPLET_WARPS, triplet_warps)
+        if g2_wide:
+            self.set_option(G3_OPT_G2_WIDE, 1)
+        self.g2_shells = 2 * self.n_r if g2_wide else self.n_r
         self.qtet_bins = int(qtet_bins or 0)
         if self.qtet_bins:
             self.set_option(G3_OPT_QTET_BINS, self.qtet_bins)
@@ -225,10 +229,11 @@ class Plan:
         return counts, g3, [int(v) for v in stats]
 
     def finalize_g2(self, stream=None):
-        """(counts2 int64-viewed-as-uint64 [n_r], g2 fp64 [n_r]) device tensors; stream-ordered."""
+        """(counts2 int64-viewed-as-uint64 [S], g2 fp64 [S]) device tensors, S = n_r, or 2 n_r with
+        g2_wide; stream-ordered."""
         import torch
-        counts2 = torch.empty(self.n_r, dtype=torch.int64, device="cuda")
-        g2 = torch.empty(self.n_r, dtype=torch.float64, device="cuda")
+        counts2 = torch.empty(self.g2_shells, dtype=torch.int64, device="cuda")
+        g2 = torch.empty(self.g2_shells, dtype=torch.float64, device="cuda")
         _check(self._lib.g3_finalize_g2(self._h, counts2.data_ptr(), g2.data_ptr(), _stream_ptr(stream)),
                "g3_finalize_g2")
         return counts2, g2

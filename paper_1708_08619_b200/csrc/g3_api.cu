@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "g3_cells.cuh"
+#include "g3_g2wide.cuh"
 #include "g3_generic.cuh"
 #include "g3_msd.cuh"
 #include "g3_plan.h"
@@ -198,6 +199,20 @@ int flush(g3_plan* p, cudaStream_t st) {
         if (rc != G3_OK) return rc;
     }
     G3_CUDA(cudaGetLastError());
+    if (p->g2_wide) {                                      // pair histogram of the shells n_r .. 2 n_r - 1
+        const double w = (p->r_max / (double)bs.n_r) * p->inv_g, eps = 1.0 / 1048576.0;
+        G2wParams gp{};
+        gp.sh.n_r = 2 * bs.n_r; gp.sh.T_r = p->d_T2; gp.sh.cut2 = p->T2.back();
+        gp.sh.cut_lo = (float)((double)p->T2.back() * (1.0 - eps));
+        gp.sh.cut_hi = (float)((double)p->T2.back() * (1.0 + eps));
+        gp.sh.inv_w_lo = (float)((1.0 / w) * (1.0 - eps));
+        gp.sh.inv_w_hi = (float)((1.0 / w) * (1.0 + eps));
+        gp.n_lo = bs.n_r; gp.counts2 = p->d_counts2;
+        const long long blocks = std::min<long long>((total + kG2wWarps - 1) / kG2wWarps, (long long)p->sm_count * 8);
+        g2_wide_kernel<<<(unsigned)blocks, kG2wWarps * 32, sizeof(uint32_t) * bs.n_r, st>>>(fb, gp);
+        p->launches += 1;
+        G3_CUDA(cudaGetLastError());
+    }
     if (p->qtet_bins > 0) {                                // q_tet on the same cell list (Eq. 1)
         const unsigned long long cw = (unsigned long long)(kGrid / p->ncell);
         QtParams qp{p->qtet_bins, (double)p->qtet_bins / 4.0, cw * cw, p->d_qtet, p->d_qtet_stats,
@@ -318,6 +333,12 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
             volatile double e2 = e * e;
             p->T_t[c] = (unsigned long long)std::ceil(e2);
         }
+        p->T2.resize(2 * bins.n_r + 1);                       // the same shells carried on to 2 r_max (g2)
+        for (int32_t b = 0; b <= 2 * bins.n_r; ++b) {
+            volatile double e = (double)b * w;
+            volatile double e2 = e * e;
+            p->T2[b] = (unsigned long long)std::ceil(e2);
+        }
     }
     // strictly increasing edges are required by bin(); they fail only for absurd bin counts
     for (size_t i = 0; i + 1 < p->T_r.size(); ++i)
@@ -339,17 +360,19 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
     G3_TRY(cudaMalloc(&p->d_T_t, sizeof(unsigned long long) * p->T_t.size()));
     G3_TRY(cudaMalloc(&p->d_counts, sizeof(unsigned long long) * p->nbins));
     G3_TRY(cudaMalloc(&p->d_stats, sizeof(unsigned long long) * 4));
-    G3_TRY(cudaMalloc(&p->d_counts2, sizeof(unsigned long long) * bins.n_r));
-    G3_TRY(cudaMemset(p->d_counts2, 0, sizeof(unsigned long long) * bins.n_r));
-    {   // shell volumes V_a = (4 pi / 3)(r_{a+1}^3 - r_a^3) for g2
-        std::vector<double> v2(bins.n_r);
+    G3_TRY(cudaMalloc(&p->d_counts2, sizeof(unsigned long long) * 2 * bins.n_r));
+    G3_TRY(cudaMemset(p->d_counts2, 0, sizeof(unsigned long long) * 2 * bins.n_r));
+    G3_TRY(cudaMalloc(&p->d_T2, sizeof(unsigned long long) * p->T2.size()));
+    G3_TRY(cudaMemcpy(p->d_T2, p->T2.data(), sizeof(unsigned long long) * p->T2.size(), cudaMemcpyHostToDevice));
+    {   // shell volumes V_a = (4 pi / 3)(r_{a+1}^3 - r_a^3) for g2, up to 2 r_max
+        std::vector<double> v2(2 * bins.n_r);
         const double w = r_max / (double)bins.n_r;
-        for (int32_t a = 0; a < bins.n_r; ++a) {
+        for (int32_t a = 0; a < 2 * bins.n_r; ++a) {
             const double r0 = a * w, r1 = (a + 1) * w;
             v2[a] = (4.0 * 3.14159265358979323846 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0);
         }
-        G3_TRY(cudaMalloc(&p->d_volumes2, sizeof(double) * bins.n_r));
-        G3_TRY(cudaMemcpy(p->d_volumes2, v2.data(), sizeof(double) * bins.n_r, cudaMemcpyHostToDevice));
+        G3_TRY(cudaMalloc(&p->d_volumes2, sizeof(double) * 2 * bins.n_r));
+        G3_TRY(cudaMemcpy(p->d_volumes2, v2.data(), sizeof(double) * 2 * bins.n_r, cudaMemcpyHostToDevice));
     }
     G3_TRY(cudaMalloc(&p->d_volumes, sizeof(double) * p->nbins));
     G3_TRY(cudaMemcpy(p->d_T_r, p->T_r.data(), sizeof(unsigned long long) * p->T_r.size(), cudaMemcpyHostToDevice));
@@ -378,6 +401,9 @@ int g3_plan_set_option(g3_plan* p, int32_t option, int64_t value) {
         case G3_OPT_TRIPLET_WARPS:
             if (value != 0 && (value < 8 || value > 24 || value % 4 != 0)) return G3_EINVAL;
             p->tri_warps_opt = (int32_t)value; break;
+        case G3_OPT_G2_WIDE:
+            if (value < 0 || value > 1) return G3_EINVAL;
+            p->g2_wide = (int32_t)value; break;
         case G3_OPT_QTET_BINS:
             if (value < 0 || value > 8192 || (value > 0 && p->n < 5)) return G3_EINVAL;
             p->qtet_bins = (int32_t)value; break;
@@ -415,6 +441,7 @@ int g3_plan_get_info(const g3_plan* cp, int32_t key, int64_t* value) {
         case G3_INFO_SM_COUNT: *value = p->sm_count; break;
         case G3_INFO_FRAMES_PENDING: *value = p->pending; break;
         case G3_INFO_SLABS: *value = p->tiled ? p->tiled->n_slabs : 0; break;
+        case G3_INFO_G2_SHELLS: *value = p->g2_wide ? 2 * p->bins.n_r : p->bins.n_r; break;
         default: return G3_EINVAL;
     }
     return G3_OK;
@@ -534,7 +561,7 @@ int g3_finalize_g2(g3_plan* p, uint64_t* d_counts2, double* d_g2, void* stream) 
     if (rc != G3_OK) return rc;
     rc = tiled_merge(p, st);
     if (rc != G3_OK) return rc;
-    const int32_t n_r = p->bins.n_r;
+    const int32_t n_r = p->g2_wide ? 2 * p->bins.n_r : p->bins.n_r;       // shells returned
     if (d_counts2)
         G3_CUDA(cudaMemcpyAsync(d_counts2, p->d_counts2, sizeof(uint64_t) * n_r, cudaMemcpyDeviceToDevice, st));
     if (d_g2) {
@@ -642,7 +669,7 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     G3_CUDA(cudaMemsetAsync(p->d_counts, 0, sizeof(unsigned long long) * p->nbins, st));
     G3_CUDA(cudaMemsetAsync(p->d_stats, 0, sizeof(unsigned long long) * 4, st));
-    G3_CUDA(cudaMemsetAsync(p->d_counts2, 0, sizeof(unsigned long long) * p->bins.n_r, st));
+    G3_CUDA(cudaMemsetAsync(p->d_counts2, 0, sizeof(unsigned long long) * 2 * p->bins.n_r, st));
     if (p->d_qtet) {
         G3_CUDA(cudaMemsetAsync(p->d_qtet, 0, sizeof(unsigned long long) * p->qtet_bins, st));
         G3_CUDA(cudaMemsetAsync(p->d_qtet_stats, 0, sizeof(unsigned long long) * 2, st));
@@ -672,7 +699,7 @@ void g3_plan_destroy(g3_plan* p) {
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
     cudaFree(p->d_T_r); cudaFree(p->d_T_t); cudaFree(p->d_counts); cudaFree(p->d_stats);
-    cudaFree(p->d_volumes); cudaFree(p->d_counts2); cudaFree(p->d_volumes2);
+    cudaFree(p->d_volumes); cudaFree(p->d_counts2); cudaFree(p->d_volumes2); cudaFree(p->d_T2);
     cudaGetLastError();
     delete p;
 }

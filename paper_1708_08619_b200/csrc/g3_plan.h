@@ -79,10 +79,13 @@ struct g3_plan {
     unsigned long long* d_T_r = nullptr;
     unsigned long long* d_T_t = nullptr;
     unsigned long long* d_counts = nullptr;  // [nbins] running histogram (ordered pairs)
-    unsigned long long* d_counts2 = nullptr; // [n_r] g2: ordered pairs (i, j) per shell of r_ij
+    unsigned long long* d_counts2 = nullptr; // [2 n_r] g2: ordered pairs (i, j) per shell of r_ij (upper half: G3_OPT_G2_WIDE)
+    unsigned long long* d_T2 = nullptr;      // [2 n_r + 1] squared shell edges b w up to 2 r_max
+    std::vector<unsigned long long> T2;
+    int32_t g2_wide = 0;                     // G3_OPT_G2_WIDE
     unsigned long long* d_stats = nullptr;   // [4]: pairs, overflow, capacity error, spare
     double* d_volumes = nullptr;             // [nbins]
-    double* d_volumes2 = nullptr;            // [n_r] shell volumes for g2
+    double* d_volumes2 = nullptr;            // [2 n_r] shell volumes for g2
     int32_t qtet_bins = 0;                   // G3_OPT_QTET_BINS: 0 = q_tet off
     unsigned long long* d_qtet = nullptr;    // [qtet_bins] histogram of q_tet on [-3, 1]
     unsigned long long* d_qtet_stats = nullptr; // [2]: atoms binned, atoms skipped
