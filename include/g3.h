@@ -59,7 +59,10 @@ extern "C" {
 typedef struct g3_plan g3_plan; /* opaque; created by g3_plan_create, freed by g3_plan_destroy */
 
 /* Bin specification.  r_ij and r_ik: n_r uniform bins on [0, r_max).
- * r_jk: n_t uniform bins on [0, 2*r_max).  1 <= n_r, n_t <= 1024. */
+ * r_jk: n_t uniform bins on [0, 2*r_max).  1 <= n_r, n_t <= 1024, and the common lattice of the
+ * r and t edges must stay below 2^19 units: 2 n_r n_t / gcd(n_t, 2 n_r) <= 524288 (the exact
+ * 128-bit bin volumes need it; n_t = n_r and n_t = 2 n_r always qualify, two coprime counts
+ * near 1024 do not: g3_plan_create then returns G3_EINVAL). */
 typedef struct {
     int32_t n_r;
     int32_t n_t;
@@ -71,7 +74,8 @@ typedef enum {
     G3_ENOMEM = 2,    /* host or device allocation failed                                   */
     G3_ECUDA = 3,     /* a CUDA runtime call failed, or no sm_100 device is present         */
     G3_ECAPACITY = 4, /* a central particle had more neighbours than the plan can hold      */
-    G3_ESTATE = 5     /* call not valid in the plan's current state                         */
+    G3_ESTATE = 5,    /* call not valid in the plan's current state                         */
+    G3_EINTERNAL = 6  /* an internal invariant failed (counts outside the histogram tile): a bug   */
 } g3_status;
 
 /* Options for g3_plan_set_option (all optional; defaults are chosen for the B200). */
@@ -136,8 +140,9 @@ G3_API int g3_plan_clear_timing(g3_plan *p);
 
 /* Add one frame (Algorithm 6/7's loop body).
  *   d_pos  device, fp64, [n][3] row-major (x,y,z of particle 0, then particle 1, ...).
- *          Any real coordinate is accepted: it is snapped to the box/2^20 grid and
- *          wrapped into the box.
+ *          Any finite coordinate is accepted: it is snapped to the box/2^20 grid and
+ *          wrapped into the box.  NaN, infinities and |x| >= 2^42 box lengths have no grid
+ *          point: they set a sticky error that g3_finalize reports as G3_EINVAL.
  * Asynchronous and stream-ordered: never synchronises the host.  d_pos is fully
  * consumed by work enqueued during this call (it is quantised into plan-owned
  * staging), so it may be reused as soon as `stream` has passed this call.  The
@@ -163,7 +168,8 @@ G3_API int g3_accumulate_frames_host(g3_plan *p, const double *h_pos, int64_t n_
  *   h_stats   host, uint64[3] = { frames, sum_i k_i (k_i - 1), overflow }; may be NULL
  * Does not reset the plan: more frames may follow, and it may be called again.
  * Errors: G3_ECAPACITY if any centre exceeded the neighbour capacity (counts are
- * then incomplete), G3_ECUDA.                                                       */
+ * then incomplete), G3_EINVAL if a non-finite coordinate was accumulated since the last
+ * reset (results meaningless), G3_EINTERNAL, G3_ECUDA.                              */
 G3_API int g3_finalize(g3_plan *p, uint64_t *d_counts, double *d_g3, uint64_t *h_stats, void *stream);
 
 /* Same with HOST output buffers (device-to-host copies included).                   */

@@ -1,5 +1,5 @@
 """g(3) triplet correlation function on one B200: Python face of the libg3 C ABI (include/g3.h)."""
-from .binding import (BENCH_EXPORTS, BENCH_LIB_PATH, EXPORTS, G3_ECAPACITY, G3_ECUDA, G3_EINVAL, G3_ENOMEM, G3_ESTATE,
+from .binding import (BENCH_EXPORTS, BENCH_LIB_PATH, EXPORTS, G3_ECAPACITY, G3_EINTERNAL, G3_ECUDA, G3_EINVAL, G3_ENOMEM, G3_ESTATE,
                       G3_INFO_BATCH_FRAMES, G3_INFO_CELLS_PER_EDGE, G3_INFO_FRAMES_PENDING,
                       G3_INFO_KERNEL, G3_INFO_KERNEL_LAUNCHES, G3_INFO_MAX_NEIGHBOURS,
                       G3_INFO_G2_SHELLS, G3_INFO_SM_COUNT, G3_INFO_SLABS, G3_INFO_TILE_BINS, G3_INFO_TIMED_LAUNCHES, G3_INFO_TRIPLET_NS,

@@ -13,7 +13,7 @@ from typing import Optional, Tuple
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libg3.so")
 
-G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE = range(6)
+G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE, G3_EINTERNAL = range(7)
 G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING, G3_OPT_TRIPLET_WARPS = 1, 2, 3, 4, 5
 G3_OPT_QTET_BINS = 6
 G3_OPT_G2_WIDE = 7

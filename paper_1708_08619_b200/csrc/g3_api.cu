@@ -69,6 +69,7 @@ void free_buffers(g3_plan* p) {
     cudaFree(p->d_cell_start); p->d_cell_start = nullptr;
     cudaFree(p->d_sorted); p->d_sorted = nullptr;
     cudaFree(p->d_sortedf); p->d_sortedf = nullptr;
+    cudaFree(p->d_generic_nb); p->d_generic_nb = nullptr;
     cudaFree(p->d_h2d); p->d_h2d = nullptr;
     cudaFree(p->d_qtet); p->d_qtet = nullptr;
     cudaFree(p->d_qtet_stats); p->d_qtet_stats = nullptr;
@@ -123,9 +124,15 @@ int configure(g3_plan* p) {
     // plans served by the generic kernel have no lists and use the 27-cell scan of g3_qtet.cuh
     p->qtet_lists = p->qtet_bins > 0 && p->kernel == 2 && (int64_t)p->batch_frames * p->n < (int64_t(1) << 31);
     if (p->kernel == 1) {
-        size_t smem = generic_smem_bytes(p->bins.n_r, p->bins.n_t, p->max_nb, kGenericWarps);
-        if (smem > (size_t)p->smem_optin) return G3_EINVAL;   // neighbour capacity too large
         G3_CUDA(allow_max_dynamic_smem(generic_triplet_kernel<kGenericWarps>, p->smem_optin));
+        p->generic_blocks = std::min<int64_t>(((int64_t)p->batch_frames * p->n + kGenericWarps - 1) / kGenericWarps,
+                                              (int64_t)p->sm_count * 32);
+        if (generic_smem_bytes(p->bins.n_r, p->bins.n_t, p->max_nb, kGenericWarps) > (size_t)p->smem_optin) {
+            // neighbour lists too long for shared memory: one global slice per warp
+            if (generic_smem_bytes(p->bins.n_r, p->bins.n_t, 0, kGenericWarps, false) > (size_t)p->smem_optin) return G3_EINVAL;
+            p->generic_blocks = std::min<int64_t>(p->generic_blocks, (int64_t)p->sm_count * 8);
+            G3_CUDA(cudaMalloc(&p->d_generic_nb, sizeof(int4) * (size_t)p->generic_blocks * kGenericWarps * p->max_nb));
+        }
     } else {
         int rc = tiled_configure(p);
         if (rc != G3_OK) return rc;
@@ -188,11 +195,10 @@ int flush(g3_plan* p, cudaStream_t st) {
     FrameBatch fb{n, F, p->ncell, nc3, p->d_sorted, p->d_sortedf, p->d_cell_start};
     BinSpec bs{p->bins.n_r, p->bins.n_t, p->d_T_r, p->d_T_t, p->T_r.back()};
     if (p->kernel == 1) {
-        size_t smem = generic_smem_bytes(bs.n_r, bs.n_t, p->max_nb, kGenericWarps);
-        long long blocks = std::min<long long>((total + kGenericWarps - 1) / kGenericWarps,
-                                               (long long)p->sm_count * 32);
+        size_t smem = generic_smem_bytes(bs.n_r, bs.n_t, p->max_nb, kGenericWarps, p->d_generic_nb == nullptr);
+        long long blocks = std::min<long long>((total + kGenericWarps - 1) / kGenericWarps, (long long)p->generic_blocks);
         generic_triplet_kernel<kGenericWarps><<<(unsigned)blocks, kGenericWarps * 32, smem, st>>>(
-            fb, bs, p->max_nb, p->d_counts, p->d_counts2, p->d_stats);
+            fb, bs, p->max_nb, p->d_generic_nb, p->d_counts, p->d_counts2, p->d_stats);
         p->launches += 1;
     } else {
         int rc = tiled_launch(p, fb, bs, st);
@@ -265,7 +271,7 @@ int accumulate_device(g3_plan* p, const double* d_pos, int64_t n_frames, int64_t
         quantise_count_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(
             d_pos + done * stride, stride, (int32_t)p->n, (int32_t)take, p->inv_g, p->ncell,
             p->d_staged + (size_t)p->pending * p->n, p->d_slot + (size_t)p->pending * p->n,
-            p->d_cell_count + (size_t)p->pending * nc3);
+            p->d_cell_count + (size_t)p->pending * nc3, p->d_stats + 4);
         p->launches += 1;
         G3_CUDA(cudaGetLastError());
         p->pending += (int32_t)take;
@@ -291,6 +297,7 @@ const char* g3_strerror(int code) {
         case G3_ECUDA: return "CUDA error or no usable sm_100 device";
         case G3_ECAPACITY: return "neighbour capacity exceeded";
         case G3_ESTATE: return "call not valid in this plan state";
+        case G3_EINTERNAL: return "internal invariant violated (histogram tile)";
         default: return "unknown status";
     }
 }
@@ -359,7 +366,7 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
     G3_TRY(cudaMalloc(&p->d_T_r, sizeof(unsigned long long) * p->T_r.size()));
     G3_TRY(cudaMalloc(&p->d_T_t, sizeof(unsigned long long) * p->T_t.size()));
     G3_TRY(cudaMalloc(&p->d_counts, sizeof(unsigned long long) * p->nbins));
-    G3_TRY(cudaMalloc(&p->d_stats, sizeof(unsigned long long) * 4));
+    G3_TRY(cudaMalloc(&p->d_stats, sizeof(unsigned long long) * 8));
     G3_TRY(cudaMalloc(&p->d_counts2, sizeof(unsigned long long) * 2 * bins.n_r));
     G3_TRY(cudaMemset(p->d_counts2, 0, sizeof(unsigned long long) * 2 * bins.n_r));
     G3_TRY(cudaMalloc(&p->d_T2, sizeof(unsigned long long) * p->T2.size()));
@@ -379,7 +386,7 @@ int g3_plan_create(g3_plan** out, int64_t n, double box, double r_max, g3_bins b
     G3_TRY(cudaMemcpy(p->d_T_t, p->T_t.data(), sizeof(unsigned long long) * p->T_t.size(), cudaMemcpyHostToDevice));
     G3_TRY(cudaMemcpy(p->d_volumes, p->volumes.data(), sizeof(double) * p->nbins, cudaMemcpyHostToDevice));
     G3_TRY(cudaMemset(p->d_counts, 0, sizeof(unsigned long long) * p->nbins));
-    G3_TRY(cudaMemset(p->d_stats, 0, sizeof(unsigned long long) * 4));
+    G3_TRY(cudaMemset(p->d_stats, 0, sizeof(unsigned long long) * 8));
 #undef G3_TRY
     *out = p;
     return G3_OK;
@@ -545,10 +552,12 @@ int g3_finalize(g3_plan* p, uint64_t* d_counts, double* d_g3, uint64_t* h_stats,
         rc = g3_normalize(p, reinterpret_cast<const uint64_t*>(p->d_counts), p->frames, d_g3, stream);
         if (rc != G3_OK) return rc;
     }
-    unsigned long long stats[4] = {0, 0, 0, 0};
+    unsigned long long stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     G3_CUDA(cudaMemcpyAsync(stats, p->d_stats, sizeof(stats), cudaMemcpyDeviceToHost, st));
     G3_CUDA(cudaStreamSynchronize(st));
     if (h_stats) { h_stats[0] = p->frames; h_stats[1] = stats[0]; h_stats[2] = stats[1]; }
+    if (stats[3]) return G3_EINTERNAL;      // counts outside the mapped tile slots: must never happen
+    if (stats[4]) return G3_EINVAL;         // NaN, infinite or absurdly large coordinates were staged
     return stats[2] ? G3_ECAPACITY : G3_OK;
 }
 
@@ -598,7 +607,7 @@ int g3_finalize_host(g3_plan* p, uint64_t* h_counts, double* h_g3, uint64_t* h_s
     double* d_g3 = nullptr;
     if (h_g3) G3_CUDA(cudaMallocAsync(&d_g3, sizeof(double) * p->nbins, st));
     int rc = g3_finalize(p, nullptr, d_g3, h_stats, stream);
-    if (rc == G3_OK || rc == G3_ECAPACITY) {
+    if (rc == G3_OK || rc == G3_ECAPACITY || rc == G3_EINVAL) {
         cudaError_t e = cudaSuccess;
         if (h_counts) e = cudaMemcpyAsync(h_counts, p->d_counts, sizeof(uint64_t) * p->nbins, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess && h_g3) e = cudaMemcpyAsync(h_g3, d_g3, sizeof(double) * p->nbins, cudaMemcpyDeviceToHost, st);
@@ -668,7 +677,7 @@ int g3_plan_reset(g3_plan* p, void* stream) {
     if (!p) return G3_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     G3_CUDA(cudaMemsetAsync(p->d_counts, 0, sizeof(unsigned long long) * p->nbins, st));
-    G3_CUDA(cudaMemsetAsync(p->d_stats, 0, sizeof(unsigned long long) * 4, st));
+    G3_CUDA(cudaMemsetAsync(p->d_stats, 0, sizeof(unsigned long long) * 8, st));
     G3_CUDA(cudaMemsetAsync(p->d_counts2, 0, sizeof(unsigned long long) * 2 * p->bins.n_r, st));
     if (p->d_qtet) {
         G3_CUDA(cudaMemsetAsync(p->d_qtet, 0, sizeof(unsigned long long) * p->qtet_bins, st));

@@ -12,9 +12,12 @@
 
 namespace g3 {
 
-__device__ __forceinline__ int32_t quantise_coord(double x, double inv_g) {
+__device__ __forceinline__ int32_t quantise_coord(double x, double inv_g, bool& bad) {
     // m = llrint(x * 2^20/box) mod 2^20; one IEEE multiply, round-to-nearest-even conversion
-    long long q = __double2ll_rn(__dmul_rn(x, inv_g));
+    const double s = __dmul_rn(x, inv_g);
+    // NaN, infinities and values the 64-bit conversion would saturate have no grid point
+    if (!(fabs(s) < 4611686018427387904.0)) bad = true;
+    long long q = __double2ll_rn(s);
     return (int32_t)(q & (kGrid - 1));
 }
 
@@ -28,15 +31,17 @@ __global__ void __launch_bounds__(256)
 quantise_count_kernel(const double* __restrict__ pos, long long frame_stride, int32_t n,
                       int32_t n_frames, double inv_g, int32_t ncell,
                       int4* __restrict__ staged, int32_t* __restrict__ slot,
-                      int32_t* __restrict__ cell_count) {
+                      int32_t* __restrict__ cell_count, unsigned long long* __restrict__ bad_count) {
     long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (long long)n_frames * n) return;
     int32_t f = (int32_t)(g / n);
     int32_t p = (int32_t)(g - (long long)f * n);
     const double* x = pos + (long long)f * frame_stride + 3ll * p;
-    int32_t mx = quantise_coord(__ldg(x + 0), inv_g);
-    int32_t my = quantise_coord(__ldg(x + 1), inv_g);
-    int32_t mz = quantise_coord(__ldg(x + 2), inv_g);
+    bool bad = false;
+    int32_t mx = quantise_coord(__ldg(x + 0), inv_g, bad);
+    int32_t my = quantise_coord(__ldg(x + 1), inv_g, bad);
+    int32_t mz = quantise_coord(__ldg(x + 2), inv_g, bad);
+    if (bad) atomicAdd(bad_count, 1ull);               // sticky: g3_finalize returns G3_EINVAL
     int32_t cell = (cell_of(mx, ncell) * ncell + cell_of(my, ncell)) * ncell + cell_of(mz, ncell);
     int32_t ncell3 = ncell * ncell * ncell;
     int32_t s = atomicAdd(cell_count + (long long)f * ncell3 + cell, 1);

@@ -1,7 +1,8 @@
 // g3_generic.cuh -- generic exact triplet kernel (kernel 1).
 //
 // Works for every plan (any bin counts, any r_max < box/2, any neighbour count up to
-// the plan's capacity).  All arithmetic that decides a bin is 64-bit integer; bins
+// the plan's capacity: the per-warp neighbour list lives in shared memory when it fits and in a
+// global-memory slice of the warp otherwise).  All arithmetic that decides a bin is 64-bit integer; bins
 // are found by binary search in the squared-edge tables; the histogram is updated
 // with 64-bit global atomics.  It is the slow, always-available path; the tiled
 // kernel (g3_tiled.cuh) is the fast one.
@@ -65,7 +66,7 @@ struct CandidateRanges {
 
 template <int kWarps>
 __global__ void __launch_bounds__(kWarps * 32)
-generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb,
+generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb, int4* nb_global,
                        unsigned long long* __restrict__ counts,
                        unsigned long long* __restrict__ counts2,
                        unsigned long long* __restrict__ stats) {
@@ -80,7 +81,8 @@ generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb,
     __syncthreads();
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    int4* nb = nb_all + (size_t)wid * max_nb;
+    // this warp's neighbour list: shared memory, or its slice of nb_global [grid][kWarps][max_nb]
+    int4* nb = nb_global ? nb_global + ((size_t)blockIdx.x * kWarps + wid) * max_nb : nb_all + (size_t)wid * max_nb;
     const long long total = (long long)fb.n_frames * fb.n;
     unsigned long long my_overflow = 0, my_pairs = 0, my_cap = 0;
 
@@ -144,9 +146,10 @@ generic_triplet_kernel(FrameBatch fb, BinSpec bs, int32_t max_nb,
     if (my_cap) atomicAdd(stats + 2, my_cap);
 }
 
-inline size_t generic_smem_bytes(int32_t n_r, int32_t n_t, int32_t max_nb, int warps) {
+// shared memory of the kernel: the edge tables, plus the lists unless they live in global memory
+inline size_t generic_smem_bytes(int32_t n_r, int32_t n_t, int32_t max_nb, int warps, bool lists_in_smem = true) {
     size_t off = ((size_t)(n_r + n_t + 2) * 8 + 15) & ~size_t(15);
-    return off + (size_t)warps * max_nb * sizeof(int4);
+    return off + (lists_in_smem ? (size_t)warps * max_nb * sizeof(int4) : 0);
 }
 
 }  // namespace g3

@@ -83,7 +83,7 @@ struct g3_plan {
     unsigned long long* d_T2 = nullptr;      // [2 n_r + 1] squared shell edges b w up to 2 r_max
     std::vector<unsigned long long> T2;
     int32_t g2_wide = 0;                     // G3_OPT_G2_WIDE
-    unsigned long long* d_stats = nullptr;   // [4]: pairs, overflow, capacity error, spare
+    unsigned long long* d_stats = nullptr;   // [8]: pairs, overflow, capacity error, internal error, bad coordinates
     double* d_volumes = nullptr;             // [nbins]
     double* d_volumes2 = nullptr;            // [2 n_r] shell volumes for g2
     int32_t qtet_bins = 0;                   // G3_OPT_QTET_BINS: 0 = q_tet off
@@ -98,6 +98,8 @@ struct g3_plan {
     int32_t* d_cell_count = nullptr;         // [batch][ncell3]
     int32_t* d_cell_start = nullptr;         // [batch][ncell3 + 1]
     int4* d_sorted = nullptr;                // [batch][n]
+    int4* d_generic_nb = nullptr;            // generic kernel: [blocks][warps][max_nb] lists when shared memory is too small
+    int64_t generic_blocks = 0;
     float4* d_sortedf = nullptr;             // [batch][n] fp32 copy of d_sorted (TMA source of the neighbour kernel)
     double* d_h2d = nullptr;                 // staging for g3_accumulate_frames_host, 2 x chunk
     cudaEvent_t h2d_done[2] = {nullptr, nullptr};   // copy of a staging half finished (copy stream)

@@ -258,6 +258,46 @@ def test_two_live_plans_of_different_shape(oracle_lib, g3):
         assert np.array_equal(c.cpu().numpy().view(np.uint64), Ho)
 
 
+def test_generic_kernel_with_lists_beyond_shared_memory(oracle_lib, g3):
+    """the paper's own cut-off r_max = L/4 on a frame large enough that neither the
+    tiled path (degenerate cell grid, n > 8192) nor the generic kernel's shared-memory list (capacity
+    ~1800) can serve it: the generic kernel keeps its lists in global memory"""
+    n, box = 9000, 10.0
+    m = uniform_frame(n, seed=2024)
+    with g3.Plan(n, box, 0.25 * box, 8, 8) as plan:
+        assert plan.info(g3.G3_INFO_KERNEL) == 1 and plan.info(g3.G3_INFO_MAX_NEIGHBOURS) > 1800
+    check(oracle_lib, g3, grid_to_pos(m, box), box, 0.25 * box, 8, 8)
+
+
+def test_non_finite_coordinates_are_an_error(g3):
+    """NaN / infinite coordinates have no grid point: sticky G3_EINVAL at finalize, cleared by reset"""
+    import torch
+    w = WORKLOADS[1]
+    _, pos = frames(w, 2)
+    d = torch.from_numpy(pos).cuda()
+    bad = d.clone()
+    bad[1, 17, 2] = float("nan")
+    bad[0, 3, 0] = float("inf")
+    for kernel in KERNELS:
+        with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, kernel=kernel) as plan:
+            plan.accumulate_frames(bad)
+            with pytest.raises(g3.G3Error) as e:
+                plan.finalize()
+            assert e.value.code == g3.G3_EINVAL
+            plan.reset()
+            plan.accumulate_frames(d)
+            plan.finalize()
+
+
+def test_bin_counts_beyond_the_volume_lattice_are_refused(g3):
+    """include/g3.h: 2 n_r n_t / gcd(n_t, 2 n_r) <= 2^19, else G3_EINVAL from g3_plan_create"""
+    with pytest.raises(g3.G3Error) as e:
+        g3.Plan(1000, 10.0, 2.0, 1021, 1023)
+    assert e.value.code == g3.G3_EINVAL
+    with g3.Plan(1000, 10.0, 2.0, 512, 512) as plan:          # equal counts always qualify
+        assert plan.info(g3.G3_INFO_KERNEL) in (1, 2)
+
+
 def test_normalize_merged_counts(oracle_lib, g3):
     """frame-sharded merge: counts from two plans summed, then g3_normalize"""
     import torch
