@@ -86,40 +86,50 @@ g2_wide_kernel(FrameBatch fb, G2wParams gp) {
                 const int32_t* __restrict__ start = fb.cell_start + (long long)f * (fb.ncell3 + 1);
                 const int32_t cell = fb.sorted[(long long)f * fb.n + s].w;
                 const int32_t cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
-                // 13 forward columns: 0..9 = ox in {1, 2} x oy in {-2..2}; 10, 11 = ox 0, oy in {1, 2}; 12 = own column
-                for (int32_t col = 0; col < 13; ++col) {
-                    const int32_t ox = col < 10 ? 1 + col / 5 : 0;
-                    const int32_t oy = col < 10 ? col % 5 - 2 : (col < 12 ? col - 9 : 0);
-                    int32_t x = cx + ox, y = cy + oy;
-                    float shx = 0.f, shy = 0.f;
-                    if (x >= nc) { x -= nc; shx = G; }
-                    if (y < 0) { y += nc; shy = -G; } else if (y >= nc) { y -= nc; shy = G; }
-                    const int32_t* __restrict__ colstart = start + (x * nc + y) * nc;
-                    const int32_t z_lo = col < 12 ? cz - 2 : cz + 1, z_hi = cz + 2;      // inclusive, before wrapping
-                    // up to three parts: cells below 0, inside, beyond nc - 1
-                    for (int part = 0; part < 3; ++part) {
-                        int32_t a, b;
-                        float shz;
-                        if (part == 0) { a = z_lo; b = min(z_hi, -1); shz = -G; if (a > b) continue; a += nc; b += nc; }
-                        else if (part == 1) { a = max(z_lo, 0); b = min(z_hi, nc - 1); shz = 0.f; if (a > b) continue; }
-                        else { a = max(z_lo, nc); b = z_hi; shz = G; if (a > b) continue; a -= nc; b -= nc; }
-                        const int32_t begin = __ldg(colstart + a), end = __ldg(colstart + b + 1);
-                        const float px = me.x - shx, py = me.y - shy, pz = me.z - shz;
-                        for (int32_t q0 = begin; q0 < end; q0 += 32) {
-                            const int32_t q = q0 + lane;
-                            const bool in = q < end;
-                            const float4 c = in ? sf[q] : me;
-                            g2w_count(c, in, px, py, pz, gp, g2w_hist);
-                        }
+                // 13 forward columns x 3 z parts (cells below 0, inside, beyond nc - 1) and the rest of the
+                // centre's own cell: 40 ranges, two per lane (slots lane and lane + 32), all fetched at once,
+                // then walked one after the other.
+                // columns 0..9 = ox in {1, 2} x oy in {-2..2}; 10, 11 = ox 0, oy in {1, 2}; 12 = own column
+                int32_t begin[2] = {0, 0}, end[2] = {0, 0};
+                float shx[2] = {0.f, 0.f}, shy[2] = {0.f, 0.f}, shz[2] = {0.f, 0.f};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int slot = lane + 32 * h;
+                    if (slot < 39) {
+                        const int32_t col = slot / 3, part = slot - 3 * col;
+                        const int32_t ox = col < 10 ? 1 + col / 5 : 0;
+                        const int32_t oy = col < 10 ? col % 5 - 2 : (col < 12 ? col - 9 : 0);
+                        int32_t x = cx + ox, y = cy + oy;
+                        if (x >= nc) { x -= nc; shx[h] = G; }
+                        if (y < 0) { y += nc; shy[h] = -G; } else if (y >= nc) { y -= nc; shy[h] = G; }
+                        const int32_t* __restrict__ colstart = start + (x * nc + y) * nc;
+                        const int32_t z_lo = col < 12 ? cz - 2 : cz + 1, z_hi = cz + 2;      // inclusive, before wrapping
+                        int32_t za, zb;
+                        if (part == 0) { za = z_lo; zb = min(z_hi, -1); shz[h] = -G; za += nc; zb += nc; }
+                        else if (part == 1) { za = max(z_lo, 0); zb = min(z_hi, nc - 1); }
+                        else { za = max(z_lo, nc); zb = z_hi; shz[h] = G; za -= nc; zb -= nc; }
+                        if (za <= zb) { begin[h] = __ldg(colstart + za); end[h] = __ldg(colstart + zb + 1); }
+                    } else if (slot == 39) {                     // the particles after the centre in its own cell
+                        begin[h] = s + 1; end[h] = __ldg(start + cell + 1);
                     }
                 }
-                // the particles after the centre in its own cell
-                const int32_t end = __ldg(start + cell + 1);
-                for (int32_t q0 = s + 1; q0 < end; q0 += 32) {
-                    const int32_t q = q0 + lane;
-                    const bool in = q < end;
-                    const float4 c = in ? sf[q] : me;
-                    g2w_count(c, in, me.x, me.y, me.z, gp, g2w_hist);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    unsigned todo = __ballot_sync(0xffffffffu, begin[h] < end[h]);
+                    while (todo) {
+                        const int src = __ffs(todo) - 1;
+                        todo &= todo - 1u;
+                        const int32_t rb = __shfl_sync(0xffffffffu, begin[h], src), re = __shfl_sync(0xffffffffu, end[h], src);
+                        const float px = me.x - __shfl_sync(0xffffffffu, shx[h], src), py = me.y - __shfl_sync(0xffffffffu, shy[h], src),
+                                    pz = me.z - __shfl_sync(0xffffffffu, shz[h], src);
+                        for (int32_t q0 = rb; q0 < re; q0 += 64) {       // two candidates per lane
+                            const int32_t qa = q0 + lane, qb = q0 + 32 + lane;
+                            const bool ina = qa < re, inb = qb < re;
+                            const float4 ca = ina ? sf[qa] : me, cb = inb ? sf[qb] : me;
+                            g2w_count(ca, ina, px, py, pz, gp, g2w_hist);
+                            g2w_count(cb, inb, px, py, pz, gp, g2w_hist);
+                        }
+                    }
                 }
             }
         }
