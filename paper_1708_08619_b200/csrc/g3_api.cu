@@ -214,8 +214,20 @@ int flush(g3_plan* p, cudaStream_t st) {
         gp.sh.inv_w_lo = (float)((1.0 / w) * (1.0 - eps));
         gp.sh.inv_w_hi = (float)((1.0 / w) * (1.0 + eps));
         gp.n_lo = bs.n_r; gp.counts2 = p->d_counts2;
-        const long long blocks = std::min<long long>((total + kG2wWarps - 1) / kG2wWarps, (long long)p->sm_count * 8);
-        g2_wide_kernel<<<(unsigned)blocks, kG2wWarps * 32, sizeof(uint32_t) * bs.n_r, st>>>(fb, gp);
+        // staged half-stencil: 64 of the 125 cells around a centre cell (1.5 x their mean occupancy)
+        const int32_t cap = (int32_t)(((int64_t)(1.5 * 64.0 * (double)p->n / (double)nc3) + 96 + 63) / 64 * 64);
+        const size_t cell_smem = g2w_cell_smem_bytes(cap, bs.n_r);
+        if (p->ncell >= 5 && cell_smem + 2048 <= (size_t)p->smem_optin) {
+            G3_CUDA(allow_max_dynamic_smem(g2_wide_cell_kernel, p->smem_optin));
+            int per_sm = 0;      // persistent: exactly the CTAs that are resident together
+            G3_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, g2_wide_cell_kernel, (kNbWarps + 1) * 32, cell_smem));
+            const long long items = (long long)nc3 * F;
+            g2_wide_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->sm_count * std::max(per_sm, 1)),
+                                  (kNbWarps + 1) * 32, cell_smem, st>>>(fb, gp, cap);
+        } else {
+            const long long blocks = std::min<long long>((total + kG2wWarps - 1) / kG2wWarps, (long long)p->sm_count * 8);
+            g2_wide_kernel<<<(unsigned)blocks, kG2wWarps * 32, sizeof(uint32_t) * bs.n_r, st>>>(fb, gp);
+        }
         p->launches += 1;
         G3_CUDA(cudaGetLastError());
     }
