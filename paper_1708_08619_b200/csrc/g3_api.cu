@@ -667,7 +667,7 @@ int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_strid
         msd_direct_kernel<<<n_blocks, kMsdWarps * 32, 0, st>>>(mp);
     }
     const double g = box / 1048576.0;
-    msd_reduce_kernel<<<(unsigned)((max_lag + 128) / 128), 128, 0, st>>>(
+    msd_reduce_kernel<<<(unsigned)((max_lag + 32) / 32), 256, 0, st>>>(
         mp.partial, n_blocks, (int32_t)max_lag, (int32_t)n, (int32_t)n_frames, g * g,
         reinterpret_cast<unsigned long long*>(d_sums), d_msd);
     if (cudaGetLastError() != cudaSuccess) return fail(G3_ECUDA);

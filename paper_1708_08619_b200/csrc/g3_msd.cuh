@@ -24,6 +24,7 @@ namespace g3 {
 
 constexpr int kMsdWarps = 16;
 constexpr int kMsdAtoms = 32;
+constexpr int kMsdLags = 8;                    // adjacent lags a warp of msd_kernel takes together
 
 struct MsdParams {
     const double* pos;                    // [F][stride] fp64, atom-major rows of 3
@@ -80,8 +81,8 @@ __device__ __forceinline__ void u128_add_s64(unsigned long long& lo, unsigned lo
 // displacement.  |m| < 2^30, so a dot product is below 3 * 2^60 and two of them fit a signed
 // 64-bit word before they are folded into a 128-bit sum; every quantity is an exact integer and
 // the result is the same 128-bit sum as the direct evaluation (reading M2).
-// A warp takes FOUR ADJACENT lags: moving the origin by one frame shifts their windows by one
-// frame, so each step loads one new origin and one new end point (6 LDS for 4 displacements).
+// A warp takes kMsdLags ADJACENT lags: moving the origin by one frame shifts their windows by one
+// frame, so each step loads one new origin and one new end point (6 LDS for kMsdLags displacements).
 __global__ void __launch_bounds__(kMsdWarps * 32)
 msd_kernel(MsdParams mp) {
     extern __shared__ __align__(16) int32_t msd_traj[];    // [F][32][3], then ulonglong2 P[F + 1]
@@ -96,12 +97,23 @@ msd_kernel(MsdParams mp) {
     {
         unsigned long long bad = 0;
         unsigned int range = 0;
-        for (int32_t t = wid; t < F; t += kMsdWarps) {
-            const double* row = mp.pos + (long long)t * mp.stride + 3ll * atom;
+        for (int32_t t0 = wid; t0 < F; t0 += 4 * kMsdWarps) {
+            double x[4][3];                                // four frames per pass: their loads are in flight together
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int32_t tu = min(t0 + u * kMsdWarps, F - 1);
+                const double* row = mp.pos + (long long)tu * mp.stride + 3ll * atom;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) x[u][c] = valid ? row[c] : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+            const int32_t t = t0 + u * kMsdWarps;
+            if (t >= F) break;                             // uniform over the warp
             int32_t m[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                m[c] = valid ? msd_snap(row[c], mp.inv_g, bad) : 0;
+                m[c] = valid ? msd_snap(x[u][c], mp.inv_g, bad) : 0;
                 msd_traj[(t * kMsdAtoms + lane) * 3 + c] = m[c];
                 range |= (unsigned int)abs(m[c]);
             }
@@ -118,6 +130,7 @@ msd_kernel(MsdParams mp) {
                 unsigned long long lo = ql, hi = 0;
                 u128_add(lo, hi, qh << 32, qh >> 32);
                 P[t + 1] = make_ulonglong2(lo, hi);
+            }
             }
         }
         if (bad) atomicAdd(mp.bad, bad);
@@ -141,58 +154,63 @@ msd_kernel(MsdParams mp) {
 
     const int32_t* base = msd_traj + lane * 3;             // element (t, this atom, c) = base[t * 96 + c]
     constexpr int32_t TS = kMsdAtoms * 3;
-    const int32_t n_groups = (mp.max_lag + 4) >> 2;        // groups of four adjacent lags
+    constexpr int L = kMsdLags;                             // adjacent lags per warp pass (a power of two)
+    const int32_t n_groups = (mp.max_lag + L) / L;
     for (int32_t grp = wid; grp < n_groups; grp += kMsdWarps) {
-        const int32_t d0 = grp << 2;
-        unsigned long long lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};
-        const int32_t n_full = F - d0 - 3;                 // origins for which all four lags exist
-        int32_t t = 0;
-        if (n_full >= 4) {
-            int32_t bx[4], by[4], bz[4];                   // b[x & 3] = r(t + d0 + x) for the four lags of a step
+        const int32_t d0 = grp * L;
+        unsigned long long lo[L], hi[L];
 #pragma unroll
-            for (int x = 0; x < 3; ++x) {
+        for (int jj = 0; jj < L; ++jj) { lo[jj] = 0; hi[jj] = 0; }
+        const int32_t n_full = F - d0 - (L - 1);           // origins for which all L lags exist
+        int32_t t = 0;
+        if (n_full >= L) {
+            int32_t bx[L], by[L], bz[L];                   // b[x & (L-1)] = r(t + d0 + x) for the L lags of a step
+#pragma unroll
+            for (int x = 0; x < L - 1; ++x) {
                 const int32_t* b = base + (d0 + x) * TS;
                 bx[x] = b[0]; by[x] = b[1]; bz[x] = b[2];
             }
-            long long acc[4] = {0, 0, 0, 0};
+            long long acc[L];
+#pragma unroll
+            for (int jj = 0; jj < L; ++jj) acc[jj] = 0;
             const int32_t* a = base;
-            const int32_t* e = base + (d0 + 3) * TS;
-#define G3_MSD_STEP(i)                                                                             \
-            {                                                                                      \
-                const int32_t ax = a[(i) * TS], ay = a[(i) * TS + 1], az = a[(i) * TS + 2];        \
-                bx[((i) + 3) & 3] = e[(i) * TS]; by[((i) + 3) & 3] = e[(i) * TS + 1]; bz[((i) + 3) & 3] = e[(i) * TS + 2]; \
-                _Pragma("unroll")                                                                  \
-                for (int jj = 0; jj < 4; ++jj)                                                     \
-                    acc[jj] += (long long)ax * bx[((i) + jj) & 3] + (long long)ay * by[((i) + jj) & 3] + \
-                               (long long)az * bz[((i) + jj) & 3];                                 \
-            }
-#define G3_MSD_FOLD()                                                                              \
-            _Pragma("unroll")                                                                      \
-            for (int jj = 0; jj < 4; ++jj) { u128_add_s64(lo[jj], hi[jj], acc[jj]); acc[jj] = 0; }
-            if (narrow) {
+            const int32_t* e = base + (d0 + L - 1) * TS;
+            // one origin: load r(t + i) and the new end point r(t + i + d0 + L - 1), L dot products
+            auto step = [&](int i) {
+                const int32_t ax = a[i * TS], ay = a[i * TS + 1], az = a[i * TS + 2];
+                bx[(i + L - 1) & (L - 1)] = e[i * TS]; by[(i + L - 1) & (L - 1)] = e[i * TS + 1]; bz[(i + L - 1) & (L - 1)] = e[i * TS + 2];
+#pragma unroll
+                for (int jj = 0; jj < L; ++jj)
+                    acc[jj] += (long long)ax * bx[(i + jj) & (L - 1)] + (long long)ay * by[(i + jj) & (L - 1)] +
+                               (long long)az * bz[(i + jj) & (L - 1)];
+            };
+            auto fold = [&]() {
+#pragma unroll
+                for (int jj = 0; jj < L; ++jj) { u128_add_s64(lo[jj], hi[jj], acc[jj]); acc[jj] = 0; }
+            };
+            if (narrow) {                                   // 32 origins per fold
                 for (; t + 32 <= n_full; t += 32) {
 #pragma unroll 1
-                    for (int u = 0; u < 8; ++u) {
-                        G3_MSD_STEP(0) G3_MSD_STEP(1) G3_MSD_STEP(2) G3_MSD_STEP(3)
-                        a += 4 * TS; e += 4 * TS;
+                    for (int u = 0; u < 32 / L; ++u) {
+#pragma unroll
+                        for (int i = 0; i < L; ++i) step(i);
+                        a += L * TS; e += L * TS;
                     }
-                    G3_MSD_FOLD()
+                    fold();
                 }
             }
-            for (; t + 4 <= n_full; t += 4) {
-                G3_MSD_STEP(0) G3_MSD_STEP(1) G3_MSD_FOLD()
-                G3_MSD_STEP(2) G3_MSD_STEP(3) G3_MSD_FOLD()
-                a += 4 * TS; e += 4 * TS;
+            for (; t + L <= n_full; t += L) {               // two origins per fold
+#pragma unroll
+                for (int i = 0; i < L; i += 2) { step(i); step(i + 1); fold(); }
+                a += L * TS; e += L * TS;
             }
-#undef G3_MSD_STEP
-#undef G3_MSD_FOLD
         }
-        // the remaining origins (fewer than four, plus those that exist only for the shorter lags)
+        // the remaining origins (fewer than L, plus those that exist only for the shorter lags)
         for (; t < F - d0; ++t) {
             const int32_t* a = base + t * TS;
             const int32_t ax = a[0], ay = a[1], az = a[2];
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj) {
+            for (int jj = 0; jj < L; ++jj) {
                 if (t + d0 + jj < F) {
                     const int32_t* b = a + (d0 + jj) * TS;
                     u128_add_s64(lo[jj], hi[jj], (long long)ax * b[0] + (long long)ay * b[1] + (long long)az * b[2]);
@@ -200,7 +218,7 @@ msd_kernel(MsdParams mp) {
             }
         }
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
+        for (int jj = 0; jj < L; ++jj) {
             const int32_t dt = d0 + jj;
             if (dt > mp.max_lag) break;                    // uniform over the warp
             unsigned long long l = lo[jj], h = hi[jj];     // cross term of this lane's atom
@@ -291,15 +309,27 @@ msd_direct_kernel(MsdParams mp) {
     }
 }
 
-// One thread per lag: add the per-CTA partials (128-bit), write (lo, hi) and msd[dt] (reading M3).
-__global__ void __launch_bounds__(128)
+// A block per 32 lags, 32 x 8 threads: thread (x, y) adds the per-CTA partials (128-bit) y, y + 8, ..
+// of lag 32 blockIdx + x (coalesced over x), the eight slices are added through shared memory,
+// and row 0 writes (lo, hi) and msd[dt] (reading M3).
+__global__ void __launch_bounds__(256)
 msd_reduce_kernel(const ulonglong2* __restrict__ partial, int32_t n_blocks, int32_t max_lag, int32_t n,
                   int32_t n_frames, double gg, unsigned long long* __restrict__ sums, double* __restrict__ msd) {
-    const int32_t dt = blockIdx.x * blockDim.x + threadIdx.x;
-    if (dt > max_lag) return;
+    __shared__ ulonglong2 slice[8][32];
+    const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
+    const int32_t dt = blockIdx.x * 32 + x;
     unsigned long long lo = 0, hi = 0;
-    for (int32_t b = 0; b < n_blocks; ++b) {
-        const ulonglong2 p = partial[(size_t)b * (max_lag + 1) + dt];
+    if (dt <= max_lag)
+        for (int32_t b = y; b < n_blocks; b += 8) {
+            const ulonglong2 p = partial[(size_t)b * (max_lag + 1) + dt];
+            lo += p.x;
+            hi += p.y + (lo < p.x ? 1ull : 0ull);
+        }
+    slice[y][x] = make_ulonglong2(lo, hi);
+    __syncthreads();
+    if (y != 0 || dt > max_lag) return;
+    for (int r = 1; r < 8; ++r) {
+        const ulonglong2 p = slice[r][x];
         lo += p.x;
         hi += p.y + (lo < p.x ? 1ull : 0ull);
     }
