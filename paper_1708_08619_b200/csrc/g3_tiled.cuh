@@ -1,5 +1,5 @@
 // g3_tiled.cuh -- the fast path (kernel 2): histogram tile layout and host-side orchestration of
-// neighbour_kernel (g3_neighbour.cuh) and tiled_triplet_kernel / merge_kernel (g3_triplet.cuh).
+// the neighbour kernels (g3_neighbour.cuh) and tiled_triplet_kernel / merge_kernel (g3_triplet.cuh).
 //
 // Tile layout.  Only bins with a <= b that the triangle inequality
 // allows get a slot:  slot(a, b, c) = 1 + BASE(b) + P(a) + c - g(b) + h(a), with
@@ -164,7 +164,7 @@ inline int32_t tiled_select(g3_plan* p) {
     if (p->max_nb > (1 << 16)) return 1;
     TiledState ts;
     if (!tiled_plan_slabs(p, ts)) return 1;
-    if ((p->ncell == 1 ? nb_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r)
+    if ((p->ncell == 1 ? nb_all_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r)
                        : nb_cell_smem_bytes(tiled_stage_cap(p), p->max_nb, p->bins.n_r, kNbStages)) + 1024 > (size_t)p->smem_optin) return 1;   // + static shared
     if (p->ncell == 1 && p->n > 8192) return 1;
     return 2;
@@ -231,7 +231,7 @@ inline int tiled_configure(g3_plan* p) {
     ts->tri_warps = tiled_warps(p, ts->slab_bins_max);
     ts->tri_smem = tri_smem_bytes(ts->slab_bins_max, ts->tri_warps, n_r);
     ts->stage_cap = tiled_stage_cap(p);
-    ts->nb_smem = p->ncell == 1 ? nb_smem_bytes(ts->stage_cap, p->max_nb, n_r)
+    ts->nb_smem = p->ncell == 1 ? nb_all_smem_bytes(ts->stage_cap, p->max_nb, n_r)
                                 : nb_cell_smem_bytes(ts->stage_cap, p->max_nb, n_r, kNbStages);
 
     std::vector<float> addend(n_r);
@@ -288,7 +288,7 @@ inline int tiled_configure(g3_plan* p) {
     G3T_CUDA(cudaMemset(ts->d_scratch, 0, sizeof(unsigned long long) * ts->tile_bins * ts->grid));
     G3T_CUDA(cudaMemset(ts->d_nbv, 0, sizeof(float4) * (per_frame_entries * B + 64)));
     if (p->ncell == 1) {
-        G3T_CUDA(allow_max_dynamic_smem(neighbour_kernel<true>, p->smem_optin));
+        G3T_CUDA(allow_max_dynamic_smem(neighbour_all_kernel, p->smem_optin));
     } else {
         auto kern = neighbour_cell_kernel<kNbStages>;
         G3T_CUDA(allow_max_dynamic_smem(kern, p->smem_optin));
@@ -350,7 +350,7 @@ inline int tiled_launch(g3_plan* p, const FrameBatch& fb, const BinSpec& bs, cud
     }
     if (fb.ncell == 1) {
         dim3 grid((unsigned)((fb.n + 63) / 64), (unsigned)fb.n_frames);
-        neighbour_kernel<true><<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
+        neighbour_all_kernel<<<grid, kNbWarps * 32, ts->nb_smem, st>>>(fb, np);
     } else {
         const long long items = (long long)fb.ncell3 * fb.n_frames;
         auto kern = neighbour_cell_kernel<kNbStages>;

@@ -2,7 +2,7 @@
 // and the merge of its per-CTA partial histograms.
 //
 // tiled_triplet_kernel: persistent, one CTA per SM, a warp per centre.  The centre's neighbour
-// list (sorted by shell, so a_j <= a_k for j < k; written by neighbour_kernel already in window
+// list (sorted by shell, so a_j <= a_k for j < k; written by the neighbour kernels already in window
 // form) is staged in a per-warp shared-memory window; every UNORDERED pair j < k is visited once
 // and counted with one shared-memory atomic into a privatised histogram tile that holds only the
 // bins the triangle inequality allows:
