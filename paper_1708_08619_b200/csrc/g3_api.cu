@@ -3,9 +3,11 @@
 // Per batch of staged frames, all stream-ordered and without host synchronisation:
 //   quantise_count_kernel   a1 + a2  snap to the 2^20 grid, cell id, rank within cell
 //   cell_scan_kernel        a2       exclusive scan of cell counts (one block per frame)
-//   cell_scatter_kernel     a2       counting-sort scatter into cell-major order
-//   triplet kernel          a3..a5   neighbours, pairs, histogram (generic or tiled)
-// and at g3_finalize:  normalise_kernel (a6).
+//   cell_scatter_kernel     a2       counting-sort scatter into cell-major order (int4 + fp32 copies)
+//   neighbour kernel        a3       shell-sorted minimum-image lists, g2 counts (tiled path)
+//   triplet kernel          a4, a5   pairs, histogram tile (tiled path); the generic kernel does a3..a5
+//   optional: g2_wide_(cell_)kernel (g2 to 2 r_max), qtet_list_kernel / qtet_cell_kernel (+ redo)
+// and at g3_finalize:  merge_kernel (a5), normalise_kernel (a6).
 #include <cuda_runtime.h>
 
 #include <algorithm>

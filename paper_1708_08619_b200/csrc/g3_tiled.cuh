@@ -1,7 +1,7 @@
 // g3_tiled.cuh -- the fast path (kernel 2): histogram tile layout and host-side orchestration of
 // the neighbour kernels (g3_neighbour.cuh) and tiled_triplet_kernel / merge_kernel (g3_triplet.cuh).
 //
-// Tile layout (DESIGN.md section 4.3).  Only bins with a <= b that the triangle inequality
+// Tile layout (DESIGN.md section 5.3).  Only bins with a <= b that the triangle inequality
 // allows get a slot:  slot(a, b, c) = 1 + BASE(b) + P(a) + c - g(b) + h(a), with
 //   g(b)  = lowest reachable c for shells (0, b),
 //   h(a)  = max_b (g(b) - c_lo(a, b))   (how far below g(b) row a can reach),
