@@ -44,6 +44,17 @@ UNIT = "triplets/s"
 WORKLOAD_INDEX = 4
 ALGO_INSTR_PER_TRIPLET = 12          # fixed algorithmic instruction count
 SM_LANES = 128                       # 4 schedulers x 32 lanes, one warp instruction per cycle each
+def ncu_lsu_busy(kernel: str):
+    """`l1tex__data_pipe_lsu_wavefronts` (% of peak) of `kernel` from its ncu summary under profiles/:
+    the shared-memory data pipe is what binds both hot kernels; None if absent."""
+    path = os.path.join(ROOT, "profiles", TRAFFIC_PROFILES.get(kernel, ""))
+    try:
+        m = re.search(r"l1tex__data_pipe_lsu_wavefronts\.avg\.pct_of_peak_sustained_elapsed`\) \| ([0-9.]+) %", open(path).read())
+    except OSError:
+        return None
+    return float(m.group(1)) / 100.0 if m else None
+
+
 ALGO_INSTR_PER_DISPLACEMENT = 9       # MSD: 3 subtractions, 3 multiply-adds, one 128-bit accumulate (DESIGN.md 6)
 ALGO_INSTR_PER_QTET_ATOM = 210        # q_tet: exact keys + top-4 insertion of ~6 list-head entries (150) + Eq. 1 in fp64 (60)
 TRAFFIC_PROFILES = {"tiled_triplet_kernel": "r2_triplet_kernel.md", "neighbour_cell_kernel": "r2_neighbour_kernel.md"}
@@ -394,6 +405,10 @@ def run_ours(args):
         "traffic_unit": f"bytes of DRAM traffic per launch (ncu --set full, {tri_traffic_src})",
         "traffic_algorithmic_bytes": alg_bytes_per_launch,
         "neighbour_kernel_traffic": nb_traffic,
+        "lsu_data_pipe_busy_ncu": {"tiled_triplet_kernel": ncu_lsu_busy("tiled_triplet_kernel"),
+                                   "neighbour_cell_kernel": ncu_lsu_busy("neighbour_cell_kernel"),
+                                   "note": "both hot kernels are bound by the shared-memory data pipe "
+                                           "(atomics + operand loads), not by issue slots: DESIGN.md 6"},
         "peak_kind": f"{sm_count} SMs x {SM_LANES} lanes x sm_max_mhz ({pk_kind}); DESIGN.md 6",
         "algorithmic_instr_per_triplet": ALGO_INSTR_PER_TRIPLET,
         "triplets_per_launch": trip_per_launch, "kernel_ms_per_launch": tri_s * 1e3,
