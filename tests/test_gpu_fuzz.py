@@ -1,0 +1,79 @@
+"""Randomised parity: seeded random shapes (particle counts, box, r_max from 2 % to 49 % of the box,
+bin counts, uniform / clumped / lattice-with-duplicates frames, with and without the wide g2
+range).  The tiled path (kernel 2 where it applies) and the generic kernel must agree bit for bit
+on counts, statistics and g2, and with the oracle wherever the case is small enough for it."""
+import numpy as np
+import pytest
+
+from workloads import GRID, grid_to_pos, uniform_frame
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def g3():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1708_08619_b200 import build
+    build.build()
+    import paper_1708_08619_b200 as g3
+    g3.load()
+    return g3
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_shapes(oracle_lib, g3, seed):
+    import torch
+    rng = np.random.default_rng(seed)
+    compared = checked_by_oracle = 0
+    for _ in range(40):
+        n = int(rng.integers(3, 6000))
+        box = float(rng.uniform(1.0, 20.0))
+        r_max = box * float(rng.uniform(0.02, 0.49))
+        n_r, n_t = int(rng.integers(1, 90)), int(rng.integers(1, 150))
+        kind = int(rng.integers(0, 3))
+        if kind == 0:
+            m = uniform_frame(n, seed=int(rng.integers(1 << 30)))
+        elif kind == 1:                                        # a blob somewhere in the box
+            m = ((rng.integers(0, GRID // int(rng.integers(2, 40)), size=(n, 3)) + rng.integers(0, GRID, size=3)) % GRID)
+        else:                                                  # coarse lattice: many exact ties and duplicates
+            m = rng.integers(0, 16, size=(n, 3)) * (GRID // 16)
+        m = m.astype(np.int32)
+        mean_k = n * 4.19 * (r_max / box) ** 3 * (8 if kind == 1 else 1)
+        if n * mean_k * mean_k > 3e9:                          # keep the work bounded
+            continue
+        F = int(rng.integers(1, 4))
+        ms = np.stack([np.roll(m, f, axis=0) for f in range(F)])
+        pos = grid_to_pos(ms, box)
+        d = torch.from_numpy(pos).cuda()
+        wide = bool(rng.integers(0, 2))
+        res = {}
+        for kernel in (1, 2):
+            try:
+                with g3.Plan(n, box, r_max, n_r, n_t, kernel=kernel, g2_wide=wide,
+                             max_neighbours=int(min(n - 1, 3 * mean_k + 200))) as plan:
+                    plan.accumulate_frames(d)
+                    c, _, st = plan.finalize(want_g3=False)
+                    c2, _ = plan.finalize_g2()
+                    res[kernel] = (c.cpu().numpy().view(np.uint64), st, c2.cpu().numpy().view(np.uint64))
+            except g3.G3Error as e:
+                res[kernel] = e.code
+        a, b = res[1], res[2]
+        if isinstance(a, int) or isinstance(b, int):           # only a capacity error may differ between kernels
+            assert a == b or g3.G3_ECAPACITY in (a, b), (a if isinstance(a, int) else "ok", b if isinstance(b, int) else "ok")
+            continue
+        case = (n, box, r_max, n_r, n_t, kind, F, wide)
+        assert np.array_equal(a[0], b[0]) and a[1] == b[1] and np.array_equal(a[2], b[2]), case
+        compared += 1
+        if n * mean_k * mean_k < 2e8:
+            orc = oracle_lib.Oracle(n, box, r_max, n_r, n_t, mode="allpairs" if n < 1500 else "cells")
+            orc.accumulate(pos)
+            Ho, _, so = orc.finalize()
+            assert np.array_equal(a[0], Ho) and a[1] == [int(v) for v in so], case
+            T = oracle_lib.thresholds(box, (2.0 if wide else 1.0) * r_max, (2 if wide else 1) * n_r, 1)[0]
+            H2 = np.zeros(T.size - 1, dtype=np.uint64)
+            for f in range(F):
+                oracle_lib.g2_frame(ms[f], T, H2)
+            assert np.array_equal(a[2], H2), case
+            checked_by_oracle += 1
+    assert compared >= 10 and checked_by_oracle >= 5
