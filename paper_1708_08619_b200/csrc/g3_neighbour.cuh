@@ -197,33 +197,25 @@ __device__ __forceinline__ void nb_scan_group(uint32_t stage_s, int32_t n_pad, i
     uint32_t sp = stage_s + ((uint32_t)lane << 4);
     const uint32_t sp_end = stage_s + ((uint32_t)n_pad << 4);
     uint32_t q = (uint32_t)lane;
-    uint32_t wr[G];                                     // write address of each list
 #pragma unroll
-    for (int g = 0; g < G; ++g) wr[g] = list_s + (uint32_t)g * list_bytes;
-    // A round adds at most 32 entries to a list: as many rounds as surely fit run without a capacity
-    // test, then the room is measured again.
-    while (sp < sp_end) {
-        uint32_t used = wr[0] - list_s;
-        if (G > 1) used = max(used, wr[1] - (list_s + list_bytes));
-        if (G > 2) used = max(used, wr[2] - (list_s + 2u * list_bytes));
-        const int32_t room = (cap - (int32_t)(used >> 1)) >> 5;
-        if (room <= 0) break;
-        const uint32_t chunk_end = min(sp_end, sp + ((uint32_t)room << 9));
-        for (; sp < chunk_end; sp += 512, q += 32) {
-            const float4 c = lds128(sp);
+    for (int g = 0; g < G; ++g) cnt[g] = 0;
+    const int32_t safe = cap - 32;                      // while 32 more entries fit, stores need no test
+    for (; sp < sp_end; sp += 512, q += 32) {
+        int32_t mx = cnt[0];
+        if (G > 1) mx = max(mx, cnt[1]);
+        if (G > 2) mx = max(mx, cnt[2]);
+        if (mx > safe) break;
+        const float4 c = lds128(sp);
 #pragma unroll
-            for (int g = 0; g < G; ++g) {
-                const float dx = c.x - p[g].x, dy = c.y - p[g].y, dz = c.z - p[g].z;
-                const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                const bool hit = d2 < cut_hi;
-                const unsigned m = __ballot_sync(0xffffffffu, hit);
-                if (hit) sts_u16(wr[g] + ((uint32_t)__popc(m & lt_mask) << 1), q);
-                wr[g] += (uint32_t)__popc(m) << 1;
-            }
+        for (int g = 0; g < G; ++g) {
+            const float dx = c.x - p[g].x, dy = c.y - p[g].y, dz = c.z - p[g].z;
+            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const bool hit = d2 < cut_hi;
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            if (hit) sts_u16(list_s + (uint32_t)g * list_bytes + ((uint32_t)(cnt[g] + __popc(m & lt_mask)) << 1), q);
+            cnt[g] += __popc(m);
         }
     }
-#pragma unroll
-    for (int g = 0; g < G; ++g) cnt[g] = (int32_t)((wr[g] - (list_s + (uint32_t)g * list_bytes)) >> 1);
     for (; sp < sp_end; sp += 512, q += 32) {           // a list is nearly full: tested stores
         const float4 c = lds128(sp);
 #pragma unroll
