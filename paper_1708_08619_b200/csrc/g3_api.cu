@@ -513,9 +513,16 @@ int g3_accumulate_frames_host(g3_plan* p, const double* h_pos, int64_t n_frames,
     // kernels of chunk c.  h2d_done[h] orders copy -> quantise kernel, h2d_free[h] orders the
     // kernels that read half h -> the next copy into it.  When the caller's stream has passed
     // this call every copy has completed, so the include/g3.h lifetime rule for h_pos holds.
+    // A long call ramps up: its first two chunks are a quarter and a half of a batch and are reduced at
+    // once, so that the GPU starts after a quarter of a batch's copy time and every later copy is hidden
+    // behind the kernels of the chunk before it.
+    const bool ramp = p->pending == 0 && n_frames >= 3 * chunk && chunk >= 8;
     int64_t done = 0;
+    int n_chunk = 0;
     while (done < n_frames) {
-        const int64_t take = std::min(chunk, n_frames - done);
+        const bool head = ramp && n_chunk < 2;
+        const int64_t take = head ? (n_chunk == 0 ? chunk / 4 : chunk / 2) : std::min(chunk, n_frames - done);
+        ++n_chunk;
         const int h = (int)(p->h2d_chunks & 1);
         double* dst = p->d_h2d + (size_t)h * chunk * 3 * p->n;
         if (p->h2d_chunks >= 2) G3_CUDA(cudaStreamWaitEvent(p->copy_stream, p->h2d_free[h], 0));
@@ -530,6 +537,7 @@ int g3_accumulate_frames_host(g3_plan* p, const double* h_pos, int64_t n_frames,
         G3_CUDA(cudaEventRecord(p->h2d_done[h], p->copy_stream));
         G3_CUDA(cudaStreamWaitEvent(st, p->h2d_done[h], 0));
         rc = accumulate_device(p, dst, take, 3 * p->n, st);
+        if (rc == G3_OK && head) rc = flush(p, st);
         if (rc != G3_OK) return rc;
         G3_CUDA(cudaEventRecord(p->h2d_free[h], st));
         p->h2d_chunks += 1;
