@@ -117,8 +117,8 @@ int configure(g3_plan* p) {
 
     if (p->batch_auto) {
         // every triplet launch zeroes and flushes a whole histogram tile per CTA (~75 us at 64^3
-        // bins): stage enough frames for ~2^21 centres per launch sequence
-        const int64_t want = ((int64_t(1) << 21) + p->n - 1) / p->n;
+        // bins): stage enough frames for ~2^22 centres per launch sequence
+        const int64_t want = ((int64_t(1) << 22) + p->n - 1) / p->n;
         p->batch_frames = (int32_t)std::min<int64_t>(std::max<int64_t>(want, 16), 256);
     }
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled

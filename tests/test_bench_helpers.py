@@ -16,11 +16,15 @@ def load_bench():
 
 def test_ncu_figures_are_found_in_profiles():
     bench = load_bench()
+    import re
     for kernel in ("tiled_triplet_kernel", "neighbour_cell_kernel"):
-        traffic, src = bench.ncu_traffic(kernel, 64)
+        path = os.path.join(ROOT, "profiles", bench.TRAFFIC_PROFILES[kernel])
+        fpl = int(re.search(r"frames_per_launch=(\d+)", open(path).read()).group(1))
+        assert fpl == 117                                  # config 4's default batch: what bench.py runs
+        traffic, src = bench.ncu_traffic(kernel, fpl)
         assert src and os.path.exists(os.path.join(ROOT, src))
-        assert traffic and 1e8 < traffic < 1e11            # bytes per 64-frame launch
-        assert bench.ncu_traffic(kernel, 63)[0] is None    # another batch size: not quoted
+        assert traffic and 1e8 < traffic < 1e11            # bytes per launch
+        assert bench.ncu_traffic(kernel, fpl - 1)[0] is None    # another batch size: not quoted
         busy = bench.ncu_lsu_busy(kernel)
         assert busy and 0.3 < busy <= 1.0
 
