@@ -75,7 +75,9 @@ typedef enum {
     G3_ECUDA = 3,     /* a CUDA runtime call failed, or no sm_100 device is present         */
     G3_ECAPACITY = 4, /* a central particle had more neighbours than the plan can hold      */
     G3_ESTATE = 5,    /* call not valid in the plan's current state                         */
-    G3_EINTERNAL = 6  /* an internal invariant failed (counts outside the histogram tile): a bug   */
+    G3_EINTERNAL = 6, /* an internal invariant failed (counts outside the histogram tile): a bug   */
+    G3_ELIMIT = 7     /* the problem needs more scratch than a no-allocation entry point owns (see
+                         g3_msd_static); nothing was computed, the allocating call still serves it */
 } g3_status;
 
 /* Options for g3_plan_set_option (all optional; defaults are chosen for the B200). */
@@ -220,6 +222,52 @@ G3_API int g3_bin_volumes(const g3_plan *p, double *h_volumes);
  * meaningless), G3_ENOMEM, G3_ECUDA.                                                       */
 G3_API int g3_msd(const double *d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
                   int64_t max_lag, uint64_t *d_sums, double *d_msd, void *stream);
+
+/* g3_msd for callers that must not allocate device memory: same arguments, same outputs (the
+ * sums are the same exact integers, bit for bit), but NO cudaMalloc / cudaMallocAsync / cudaFree or
+ * any other allocating routine is called, on any call.
+ *
+ * Who needs it.  g3_msd takes its scratch (one 128-bit partial sum per (block of 32 atoms, lag) and
+ * an error counter) from the stream's memory pool on every call.  That is a driver allocation
+ * outside whatever allocator the host program runs, and some host programs cannot afford one:
+ *   - an MD engine or a PyTorch job that analyses in situ and has already handed (nearly) all of
+ *     HBM to its own pool or caching allocator: the driver then has nothing left to give, and
+ *     g3_msd fails with G3_ENOMEM although the program itself still shows plenty of free memory;
+ *   - a job that runs under a fixed per-process memory limit (MPS partition, batch-system quota)
+ *     sized from its start-up footprint, where any later growth is a hard failure;
+ *   - an analysis step between time steps that must cost the same on every call: a pool that has
+ *     to grow goes to the driver for memory, which is slow and is one more thing that can fail.
+ * Such callers pre-allocate d_pos / d_sums / d_msd themselves, once, and call this function.
+ *
+ * How.  The scratch is a fixed array compiled into libg3 (device memory with static storage:
+ * G3_MSD_STATIC_SCRATCH_BYTES, about 8 MiB).  Every GPU on which libg3's kernels get loaded
+ * holds that array from then until the process exits, whether or not this function is used.
+ *
+ * Limits (G3_ELIMIT beyond them, before any device work; g3_msd has neither limit):
+ *   - ceil(n / 32) * (max_lag + 1) <= G3_MSD_STATIC_MAX_PARTIALS (the config-4 shape, n = 32768
+ *     with 500 lags, fits: 512000);
+ *   - the trajectories of 32 atoms must fit the shared memory of one SM: 400 n_frames + 16 bytes
+ *     <= the device's opt-in limit (n_frames <= 580 on a B200).  Longer runs need the snapped
+ *     global copy of g3_msd, which is far too large for a built-in array.
+ *
+ * First call on each device: looks up the device address of the built-in array, with that device
+ * current, and caches it per device (thread-safe).  This may load libg3's kernels onto the GPU,
+ * which is where the driver places the array.  Make this first call early, during set-up, and
+ * before any stream capture is started.  Later calls on that device touch no set-up code.
+ *
+ * Sharing.  All calls in the process, from all threads and streams, use the ONE array of their
+ * device, and it keeps whatever the previous call left in it.  Each call clears the error counter
+ * itself and overwrites every partial sum before reading it, so calls that follow each other
+ * are independent; two calls whose GPU work overlaps in time (different streams, or threads that
+ * do not order their calls) race on the array and give wrong sums without any error.  The
+ * caller serialises them.  g3_msd is not affected: it never touches the array.
+ *
+ * Stream-ordered work, then SYNCHRONISES `stream`, like g3_msd.
+ * Errors: G3_EINVAL and G3_ECUDA as g3_msd; G3_ELIMIT (see above).                              */
+#define G3_MSD_STATIC_MAX_PARTIALS 524288
+#define G3_MSD_STATIC_SCRATCH_BYTES (256 + 16 * G3_MSD_STATIC_MAX_PARTIALS)
+G3_API int g3_msd_static(const double *d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
+                         int64_t max_lag, uint64_t *d_sums, double *d_msd, void *stream);
 
 /* Zero the histogram, frame count and error state; keep all buffers.                */
 G3_API int g3_plan_reset(g3_plan *p, void *stream);

@@ -13,7 +13,7 @@ from typing import Optional, Tuple
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libg3.so")
 
-G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE, G3_EINTERNAL = range(7)
+G3_OK, G3_EINVAL, G3_ENOMEM, G3_ECUDA, G3_ECAPACITY, G3_ESTATE, G3_EINTERNAL, G3_ELIMIT = range(8)
 G3_OPT_BATCH_FRAMES, G3_OPT_KERNEL, G3_OPT_MAX_NEIGHBOURS, G3_OPT_TIMING, G3_OPT_TRIPLET_WARPS = 1, 2, 3, 4, 5
 G3_OPT_QTET_BINS = 6
 G3_OPT_G2_WIDE = 7
@@ -25,7 +25,7 @@ EXPORTS = [
     "g3_plan_create", "g3_plan_set_option", "g3_plan_get_info", "g3_plan_clear_timing",
     "g3_accumulate_frame",
     "g3_accumulate_frames", "g3_accumulate_frames_host", "g3_finalize", "g3_finalize_host",
-    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_msd", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
+    "g3_finalize_g2", "g3_finalize_qtet", "g3_normalize", "g3_bin_volumes", "g3_msd", "g3_msd_static", "g3_plan_reset", "g3_plan_destroy", "g3_strerror",
 ]
 
 
@@ -66,6 +66,7 @@ def load() -> C.CDLL:
     lib.g3_normalize.argtypes = [vp, vp, C.c_uint64, vp, vp]
     lib.g3_bin_volumes.argtypes = [vp, vp]
     lib.g3_msd.argtypes = [vp, i64, i64, i64, f64, i64, vp, vp, vp]
+    lib.g3_msd_static.argtypes = [vp, i64, i64, i64, f64, i64, vp, vp, vp]
     lib.g3_plan_reset.argtypes = [vp, vp]
     lib.g3_plan_destroy.argtypes = [vp]
     lib.g3_plan_destroy.restype = None
@@ -134,6 +135,36 @@ def msd(d_pos, box: float, max_lag: Optional[int] = None, stream=None):
     out = torch.empty(L + 1, dtype=torch.float64, device="cuda")
     _check(load().g3_msd(d_pos.data_ptr(), F, n, 3 * n, float(box), L, sums.data_ptr(), out.data_ptr(),
                          _stream_ptr(stream)), "g3_msd")
+    return sums, out
+
+
+G3_MSD_STATIC_MAX_PARTIALS = 524288           # include/g3.h
+
+
+def msd_static(d_pos, box: float, max_lag: Optional[int] = None, stream=None, sums=None, out=None):
+    """g3_msd_static: msd() for programs that must not allocate device memory (see include/g3.h:
+    their own allocator owns the GPU's memory, or they run under a fixed memory limit).  The
+    library's scratch is a fixed built-in array, so the C call allocates nothing; pass `sums`
+    (int64 cuda [max_lag+1, 2]) and `out` (float64 cuda [max_lag+1]) tensors created beforehand and
+    this wrapper allocates nothing either.  Raises G3Error with code G3_ELIMIT when
+    ceil(n/32) * (max_lag+1) > G3_MSD_STATIC_MAX_PARTIALS or the run has more than ~580 frames.
+    Calls on one GPU share the array: do not let two of them overlap on the device."""
+    import torch
+    if d_pos.dtype != torch.float64 or d_pos.device.type != "cuda" or not d_pos.is_contiguous() or \
+            d_pos.dim() != 3 or d_pos.shape[2] != 3:
+        raise ValueError("positions must be a contiguous float64 cuda tensor [F, n, 3]")
+    F, n = int(d_pos.shape[0]), int(d_pos.shape[1])
+    L = F - 1 if max_lag is None else int(max_lag)
+    if sums is None:
+        sums = torch.empty((L + 1, 2), dtype=torch.int64, device="cuda")
+    if out is None:
+        out = torch.empty(L + 1, dtype=torch.float64, device="cuda")
+    if sums.dtype != torch.int64 or out.dtype != torch.float64 or sums.device.type != "cuda" or \
+            out.device.type != "cuda" or not sums.is_contiguous() or not out.is_contiguous() or \
+            sums.numel() < 2 * (L + 1) or out.numel() < L + 1:
+        raise ValueError("sums must be int64 cuda [max_lag+1, 2] and out float64 cuda [max_lag+1], contiguous")
+    _check(load().g3_msd_static(d_pos.data_ptr(), F, n, 3 * n, float(box), L, sums.data_ptr(), out.data_ptr(),
+                                _stream_ptr(stream)), "g3_msd_static")
     return sums, out
 
 

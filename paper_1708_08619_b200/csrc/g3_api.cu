@@ -14,6 +14,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -312,6 +313,7 @@ const char* g3_strerror(int code) {
         case G3_ECAPACITY: return "neighbour capacity exceeded";
         case G3_ESTATE: return "call not valid in this plan state";
         case G3_EINTERNAL: return "internal invariant violated (histogram tile)";
+        case G3_ELIMIT: return "problem exceeds the built-in scratch of a no-allocation entry point";
         default: return "unknown status";
     }
 }
@@ -687,6 +689,99 @@ int g3_msd(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_strid
     cudaFreeAsync(ws, st);
     if (bad) rc = G3_EINVAL;              // coordinates outside +-2^30 grid units: results invalid
     return rc;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// g3_msd_static: g3_msd without any device allocation (include/g3.h says who needs that and why).
+// The scratch of msd_kernel / msd_reduce_kernel -- the per-(CTA, lag) 128-bit partial sums and the
+// bad-coordinate counter -- lives in the array below instead of in memory from the stream's pool.
+// The kernels are the ones g3_msd launches, so the sums are the same integers.
+//
+// The array has static storage on the device: the driver creates one copy per GPU when this
+// library's kernels are loaded there, and it stays until the process ends.  Layout: bytes [0, 8)
+// the bad-coordinate counter, bytes [256, 256 + 16 * kMsdStaticPartials) the partial sums.
+//
+// NOTE for whoever edits this: in HOST code the name `g3_msd_static_scratch` is only a handle for
+// the runtime's symbol table, not a device pointer.  Passing it (or its address) to a kernel
+// compiles, and the kernel then faults or, on systems where the GPU can read host memory, quietly
+// works on the wrong bytes.  Host code gets the real address from cudaGetSymbolAddress, once per
+// device, with that device current (msd_static_scratch_ptr below).
+constexpr size_t kMsdStaticHeader = 256;
+constexpr size_t kMsdStaticPartials = G3_MSD_STATIC_MAX_PARTIALS;
+static_assert(G3_MSD_STATIC_SCRATCH_BYTES == kMsdStaticHeader + sizeof(ulonglong2) * kMsdStaticPartials,
+              "include/g3.h states the size of the built-in scratch");
+static __device__ __align__(256) unsigned char g3_msd_static_scratch[G3_MSD_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMsdStaticMaxDevices = 64;
+std::mutex g_msd_static_mutex;
+unsigned char* g_msd_static_ptr[kMsdStaticMaxDevices] = {};     // device address of the array, per GPU
+
+// One-time set-up per device; `dev` must be the current device (the symbol is resolved in the
+// current device's context).  No allocation of ours: the array already exists once the module is
+// loaded, and loading it is what the first lookup may trigger.
+int msd_static_scratch_ptr(int dev, unsigned char** out) {
+    if (dev < 0 || dev >= kMsdStaticMaxDevices) return G3_ECUDA;
+    std::lock_guard<std::mutex> lock(g_msd_static_mutex);
+    if (!g_msd_static_ptr[dev]) {
+        unsigned char* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g3_msd_static_scratch);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return G3_ECUDA;
+        }
+        g_msd_static_ptr[dev] = ptr;
+    }
+    *out = g_msd_static_ptr[dev];
+    return G3_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int g3_msd_static(const double* d_pos, int64_t n_frames, int64_t n, int64_t frame_stride, double box,
+                  int64_t max_lag, uint64_t* d_sums, double* d_msd, void* stream) {
+    if (!d_pos || n_frames < 1 || n < 1 || n > (int64_t(1) << 30) || n_frames > (int64_t(1) << 24) ||
+        frame_stride < 3 * n || !(box > 0.0) || !std::isfinite(box) || max_lag < 0 || max_lag > n_frames - 1)
+        return G3_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, cc_major = 0, smem_optin = 0;
+    G3_CUDA(cudaGetDevice(&dev));
+    G3_CUDA(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    G3_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    if (cc_major < 10) return G3_ECUDA;
+    // the two limits of the built-in scratch, checked before anything is enqueued
+    const int64_t n_blocks = (n + kMsdAtoms - 1) / kMsdAtoms;
+    const size_t traj_smem = (size_t)n_frames * kMsdAtoms * 3 * sizeof(int32_t) + (size_t)(n_frames + 1) * sizeof(ulonglong2);
+    if (traj_smem > (size_t)smem_optin) return G3_ELIMIT;                  // would need the global snapped copy
+    if (n_blocks * (max_lag + 1) > (int64_t)kMsdStaticPartials) return G3_ELIMIT;
+    unsigned char* ws = nullptr;
+    int rc = msd_static_scratch_ptr(dev, &ws);
+    if (rc != G3_OK) return rc;
+    MsdParams mp;
+    mp.pos = d_pos; mp.stride = frame_stride; mp.n = (int32_t)n; mp.n_frames = (int32_t)n_frames;
+    mp.max_lag = (int32_t)max_lag; mp.inv_g = 1048576.0 / box; mp.snapped = nullptr;
+    mp.bad = reinterpret_cast<unsigned long long*>(ws);
+    mp.partial = reinterpret_cast<ulonglong2*>(ws + kMsdStaticHeader);
+    // The array still holds the previous call's contents.  The counter is the only word that is
+    // accumulated into, so it is cleared here; every partial sum the reduce kernel reads,
+    // [n_blocks][max_lag + 1], is written by msd_kernel in this call (each CTA stores all its lags).
+    G3_CUDA(cudaMemsetAsync(mp.bad, 0, sizeof(unsigned long long), st));
+    G3_CUDA(allow_max_dynamic_smem(msd_kernel, smem_optin));
+    msd_kernel<<<(unsigned)n_blocks, kMsdWarps * 32, traj_smem, st>>>(mp);
+    const double g = box / 1048576.0;
+    msd_reduce_kernel<<<(unsigned)((max_lag + 32) / 32), 256, 0, st>>>(
+        mp.partial, (int32_t)n_blocks, (int32_t)max_lag, (int32_t)n, (int32_t)n_frames, g * g,
+        reinterpret_cast<unsigned long long*>(d_sums), d_msd);
+    G3_CUDA(cudaGetLastError());
+    unsigned long long bad = 0;
+    G3_CUDA(cudaMemcpyAsync(&bad, mp.bad, sizeof(bad), cudaMemcpyDeviceToHost, st));
+    G3_CUDA(cudaStreamSynchronize(st));
+    return bad ? G3_EINVAL : G3_OK;       // coordinates outside +-2^30 grid units: results invalid
 }
 
 int g3_bin_volumes(const g3_plan* p, double* h_volumes) {
