@@ -197,7 +197,12 @@ G3_API int g3_finalize_g2(g3_plan *p, uint64_t *d_counts2, double *d_g2, void *s
  * Reduces all staged frames, then copies the histogram and SYNCHRONISES `stream`.
  *   d_hist   device, uint64 [n_q]; may be NULL
  *   h_stats  host, uint64[2] = { atoms binned, atoms skipped }; may be NULL
- * Errors: G3_ESTATE if the option is off.                                                  */
+ * Errors: G3_ESTATE if the option is off; G3_EINVAL if a non-finite coordinate was accumulated
+ * since the last reset; G3_ECAPACITY if a centre exceeded the neighbour capacity on the tiled path
+ * (kernel 2), where q_tet is read off the same capacity-limited neighbour lists: the four nearest
+ * of such a centre may be missing and the histogram is not to be used (raise
+ * G3_OPT_MAX_NEIGHBOURS).  Plans served by the generic kernel scan the cells for q_tet and do not
+ * depend on the capacity.                                                                   */
 G3_API int g3_finalize_qtet(g3_plan *p, uint64_t *d_hist, uint64_t *h_stats, void *stream);
 
 /* Normalise externally merged counts (e.g. the sum over ranks of a frame-sharded

@@ -618,10 +618,15 @@ int g3_finalize_qtet(g3_plan* p, uint64_t* d_hist, uint64_t* h_stats, void* stre
     if (rc != G3_OK) return rc;
     if (d_hist)
         G3_CUDA(cudaMemcpyAsync(d_hist, p->d_qtet, sizeof(uint64_t) * p->qtet_bins, cudaMemcpyDeviceToDevice, st));
-    unsigned long long stats[2] = {0, 0};
+    unsigned long long stats[2] = {0, 0}, plan_stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     G3_CUDA(cudaMemcpyAsync(stats, p->d_qtet_stats, sizeof(stats), cudaMemcpyDeviceToHost, st));
+    G3_CUDA(cudaMemcpyAsync(plan_stats, p->d_stats, sizeof(plan_stats), cudaMemcpyDeviceToHost, st));
     G3_CUDA(cudaStreamSynchronize(st));
     if (h_stats) { h_stats[0] = stats[0]; h_stats[1] = stats[1]; }
+    if (plan_stats[4]) return G3_EINVAL;    // NaN, infinite or absurdly large coordinates were staged
+    // q_tet read off the neighbour lists: a list cut at the capacity is cut in scan order, not by
+    // distance, so the four nearest may be among the dropped entries
+    if (plan_stats[2] && p->qtet_lists) return G3_ECAPACITY;
     return G3_OK;
 }
 

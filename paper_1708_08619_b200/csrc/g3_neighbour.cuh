@@ -627,7 +627,9 @@ neighbour_cell_kernel(FrameBatch fb, NbParams np) {
                     const uint32_t lst = list_s + (uint32_t)g * list_bytes;
                     const float4 pc = p[g];
                     int32_t count = cnt[g];
-                    if (count > cap) { my_cap += 1; count = cap; }
+                    // overflow: the centre itself may be among the dropped hits, so that all cap kept
+                    // entries could be neighbours; max_nb of them at most fit this centre's row
+                    if (count > cap) { my_cap += 1; count = max_nb; }
                     const long long row = ((long long)f * fb.n + s) * max_nb;
                     float4* __restrict__ dst = np.nbv + row;
                     uint32_t* __restrict__ dstj = np.nbj + row;

@@ -121,3 +121,44 @@ def test_option_errors(g3):
         assert e.value.code == g3.G3_ESTATE
     with pytest.raises(g3.G3Error):
         g3.Plan(4, 10.0, 1.0, 8, 8, qtet_bins=10)
+
+
+def test_capacity_error_reaches_finalize_qtet(oracle_lib, g3):
+    """On the tiled path q_tet is read off the capacity-limited neighbour lists: a clumped frame with
+    max_neighbours = 64 cuts lists in scan order, the four nearest may be gone, and finalize_qtet
+    must say so (G3_ECAPACITY) instead of returning a histogram.  The generic kernel's q_tet scans
+    the cells and does not depend on the capacity: it still matches the oracle."""
+    import torch
+    rng = np.random.default_rng(17)
+    m = uniform_frame(6000, seed=3)
+    m[:400] = ((rng.integers(0, GRID // 64, size=(400, 3)) + GRID // 3) % GRID).astype(np.int32)   # a blob
+    pos = torch.from_numpy(grid_to_pos(m[None], 10.0)).cuda()
+    with g3.Plan(6000, 10.0, 1.2, 16, 16, qtet_bins=50, max_neighbours=64, kernel=2) as plan:
+        assert plan.info(g3.G3_INFO_KERNEL) == 2
+        plan.accumulate_frames(pos)
+        with pytest.raises(g3.G3Error) as e:
+            plan.finalize_qtet()
+        assert e.value.code == g3.G3_ECAPACITY
+    with g3.Plan(6000, 10.0, 1.2, 16, 16, qtet_bins=50, max_neighbours=64, kernel=1) as plan:
+        plan.accumulate_frames(pos)
+        hist, stats = plan.finalize_qtet()
+        with pytest.raises(g3.G3Error):
+            plan.finalize()                                     # the g(3) counts ARE incomplete
+    Ho, so = oracle_qtet(oracle_lib, [m], 50)
+    assert stats == so and np.array_equal(hist.cpu().numpy().view(np.uint64), Ho)
+    # with room for every neighbour the tiled path gives the same histogram
+    with g3.Plan(6000, 10.0, 1.2, 16, 16, qtet_bins=50, max_neighbours=1024, kernel=2) as plan:
+        plan.accumulate_frames(pos)
+        hist, stats = plan.finalize_qtet()
+    assert stats == so and np.array_equal(hist.cpu().numpy().view(np.uint64), Ho)
+
+
+def test_non_finite_coordinate_reaches_finalize_qtet(g3):
+    import torch
+    pos = torch.from_numpy(grid_to_pos(uniform_frame(500, seed=9)[None], 5.0)).cuda()
+    pos[0, 17, 1] = float("nan")
+    with g3.Plan(500, 5.0, 1.0, 8, 8, qtet_bins=20) as plan:
+        plan.accumulate_frames(pos)
+        with pytest.raises(g3.G3Error) as e:
+            plan.finalize_qtet()
+        assert e.value.code == g3.G3_EINVAL
