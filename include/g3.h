@@ -82,8 +82,13 @@ typedef enum {
 
 /* Options for g3_plan_set_option (all optional; defaults are chosen for the B200). */
 typedef enum {
-    G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1);
-                                default: max(16, 2^19 / n) capped at 256 and by memory       */
+    G3_OPT_BATCH_FRAMES = 1, /* frames staged before one batched launch sequence (>= 1); default:
+                                max(16, 2^22 / n) capped at 256, and so that the neighbour lists of
+                                a batch take at most 16 GiB and at most a quarter of the device
+                                memory free when the first frame arrives.  Whether chosen or
+                                default, the batch is halved until the plan's buffers can be
+                                allocated: it changes no result (G3_INFO_BATCH_FRAMES = the value
+                                in use)                                                         */
     G3_OPT_KERNEL = 2,       /* 0 = auto, 1 = generic exact kernel, 2 = tiled fast kernel    */
     G3_OPT_MAX_NEIGHBOURS = 3, /* per-centre neighbour capacity (0 = derive from density)    */
     G3_OPT_TRIPLET_WARPS = 5, /* warps per triplet-kernel CTA: 0 = auto, or 8, 12, .. 24  */
@@ -92,7 +97,9 @@ typedef enum {
                                 frames are accumulated; 0 (default) = off; needs n >= 5      */
     G3_OPT_G2_WIDE = 7,      /* 1 = the pair histogram g2 also covers [r_max, 2 r_max), the rest of the
                                 r_jk axis of g(3), in n_r more shells of the same width (a second
-                                pair search per frame); 0 (default) = the neighbour range only */
+                                pair search per frame over eight times the volume: it about
+                                DOUBLES the time of a step, +26 ms on the 27.5 ms of config 4);
+                                0 (default) = the neighbour range only                        */
     G3_OPT_TIMING = 4         /* 1 = bracket the neighbour and triplet kernels with CUDA events
                                  on the caller's stream (read back with g3_plan_get_info)     */
 } g3_option;

@@ -98,8 +98,7 @@ int fold_timing(g3_plan* p) {
 }
 
 // Choose the cell grid, the neighbour capacity and the kernel; allocate batch buffers.
-int configure(g3_plan* p) {
-    if (p->configured) return G3_OK;
+int configure_once(g3_plan* p) {
     const double cut = std::sqrt((double)p->T_r.back());
     const int64_t reach = (int64_t)std::ceil(cut) + 1;     // > any neighbour |component|
     int64_t ncell = kGrid / reach;                         // cell width >= reach
@@ -122,6 +121,7 @@ int configure(g3_plan* p) {
         const int64_t want = ((int64_t(1) << 22) + p->n - 1) / p->n;
         p->batch_frames = (int32_t)std::min<int64_t>(std::max<int64_t>(want, 16), 256);
     }
+    p->batch_frames = std::min(p->batch_frames, p->batch_limit);
     p->kernel = tiled_select(p);                           // 1 = generic, 2 = tiled
     // q_tet straight from the shell-sorted neighbour lists of the tiled path (qtet_list_kernel);
     // plans served by the generic kernel have no lists and use the 27-cell scan of g3_qtet.cuh
@@ -134,6 +134,10 @@ int configure(g3_plan* p) {
             // neighbour lists too long for shared memory: one global slice per warp
             if (generic_smem_bytes(p->bins.n_r, p->bins.n_t, 0, kGenericWarps, false) > (size_t)p->smem_optin) return G3_EINVAL;
             p->generic_blocks = std::min<int64_t>(p->generic_blocks, (int64_t)p->sm_count * 8);
+            // max_nb may be as large as n - 1 or 2^20: the pool of slices stays below 2 GiB (the
+            // kernel walks the centres with a grid stride, so fewer blocks only run longer)
+            const int64_t block_bytes = (int64_t)sizeof(int4) * kGenericWarps * p->max_nb;
+            p->generic_blocks = std::max<int64_t>(1, std::min<int64_t>(p->generic_blocks, (int64_t(2) << 30) / block_bytes));
             G3_CUDA(cudaMalloc(&p->d_generic_nb, sizeof(int4) * (size_t)p->generic_blocks * kGenericWarps * p->max_nb));
         }
     } else {
@@ -179,8 +183,34 @@ int configure(g3_plan* p) {
             }
         }
     }
+    if (p->g2_wide) {
+        // staged half-stencil: 64 of the 125 cells around a centre cell (1.5 x their mean occupancy)
+        p->g2w_cap = (int32_t)(((int64_t)(1.5 * 64.0 * (double)p->n / (double)nc3) + 96 + 63) / 64 * 64);
+        p->g2w_smem = g2w_cell_smem_bytes(p->g2w_cap, p->bins.n_r);
+        p->g2w_grid = 0;
+        if (p->ncell >= 5 && p->g2w_smem + 2048 <= (size_t)p->smem_optin) {
+            G3_CUDA(allow_max_dynamic_smem(g2_wide_cell_kernel, p->smem_optin));
+            int per_sm = 0;      // persistent: exactly the CTAs that are resident together
+            G3_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, g2_wide_cell_kernel, (kNbWarps + 1) * 32, p->g2w_smem));
+            p->g2w_grid = p->sm_count * std::max(per_sm, 1);
+        }
+    }
     p->configured = true;
     return G3_OK;
+}
+
+// The batch size changes no result, only how many frames share one launch sequence: when device
+// memory is short (another plan, a co-resident simulation) the batch is halved until the buffers fit.
+int configure(g3_plan* p) {
+    if (p->configured) return G3_OK;
+    p->batch_limit = INT32_MAX;
+    for (;;) {
+        const int rc = configure_once(p);
+        if (rc == G3_OK) return rc;
+        free_buffers(p);
+        if (rc != G3_ENOMEM || p->batch_frames <= 1) return rc;
+        p->batch_limit = std::max(1, p->batch_frames / 2);
+    }
 }
 
 // Reduce the staged frames into the histogram.
@@ -217,16 +247,10 @@ int flush(g3_plan* p, cudaStream_t st) {
         gp.sh.inv_w_lo = (float)((1.0 / w) * (1.0 - eps));
         gp.sh.inv_w_hi = (float)((1.0 / w) * (1.0 + eps));
         gp.n_lo = bs.n_r; gp.counts2 = p->d_counts2;
-        // staged half-stencil: 64 of the 125 cells around a centre cell (1.5 x their mean occupancy)
-        const int32_t cap = (int32_t)(((int64_t)(1.5 * 64.0 * (double)p->n / (double)nc3) + 96 + 63) / 64 * 64);
-        const size_t cell_smem = g2w_cell_smem_bytes(cap, bs.n_r);
-        if (p->ncell >= 5 && cell_smem + 2048 <= (size_t)p->smem_optin) {
-            G3_CUDA(allow_max_dynamic_smem(g2_wide_cell_kernel, p->smem_optin));
-            int per_sm = 0;      // persistent: exactly the CTAs that are resident together
-            G3_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, g2_wide_cell_kernel, (kNbWarps + 1) * 32, cell_smem));
+        if (p->g2w_grid > 0) {                             // stage capacity, shared memory and grid: see configure_once
             const long long items = (long long)nc3 * F;
-            g2_wide_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->sm_count * std::max(per_sm, 1)),
-                                  (kNbWarps + 1) * 32, cell_smem, st>>>(fb, gp, cap);
+            g2_wide_cell_kernel<<<(unsigned)std::min<long long>(items, (long long)p->g2w_grid),
+                                  (kNbWarps + 1) * 32, p->g2w_smem, st>>>(fb, gp, p->g2w_cap);
         } else {
             const long long blocks = std::min<long long>((total + kG2wWarps - 1) / kG2wWarps, (long long)p->sm_count * 8);
             g2_wide_kernel<<<(unsigned)blocks, kG2wWarps * 32, sizeof(uint32_t) * bs.n_r, st>>>(fb, gp);

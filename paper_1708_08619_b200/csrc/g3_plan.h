@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <climits>
 #include <vector>
 
 #include "../../include/g3.h"
@@ -65,7 +66,8 @@ struct g3_plan {
 
     // options / derived
     int32_t batch_frames = 16;               // frames per launch sequence (see batch_auto)
-    bool batch_auto = true;                  // derive batch_frames from n: >= 2^19 centres per launch
+    bool batch_auto = true;                  // derive batch_frames from n: ~2^22 centres per launch sequence
+    int32_t batch_limit = INT32_MAX;         // configure(): upper bound after an allocation failed (halved per retry)
     int32_t kernel_opt = 0;                  // G3_OPT_KERNEL
     int32_t kernel = 1;                      // selected kernel
     int32_t ncell = 1;
@@ -83,6 +85,9 @@ struct g3_plan {
     unsigned long long* d_T2 = nullptr;      // [2 n_r + 1] squared shell edges b w up to 2 r_max
     std::vector<unsigned long long> T2;
     int32_t g2_wide = 0;                     // G3_OPT_G2_WIDE
+    int32_t g2w_cap = 0;                     // g2_wide_cell_kernel: entries per staged half stencil,
+    size_t g2w_smem = 0;                     //   its dynamic shared memory and its persistent grid
+    int32_t g2w_grid = 0;                    //   (0 = the warp-per-centre g2_wide_kernel serves this plan)
     unsigned long long* d_stats = nullptr;   // [8]: pairs, overflow, capacity error, internal error, bad coordinates
     double* d_volumes = nullptr;             // [nbins]
     double* d_volumes2 = nullptr;            // [2 n_r] shell volumes for g2

@@ -223,9 +223,18 @@ inline int tiled_configure(g3_plan* p) {
     ts->max_batch_frames = (int64_t)((long double)ts->grid * ts->cta_item_cap * kItemCentres / (long double)p->n);
     if (ts->max_batch_frames < 1) return G3_EINVAL;
     if (p->batch_frames > ts->max_batch_frames) p->batch_frames = (int32_t)ts->max_batch_frames;
-    // neighbour lists of one batch: keep them below ~16 GiB
+    // neighbour lists of one batch: keep them below ~16 GiB, and, when the batch size is the
+    // library's own choice, below a quarter of the memory that is free right now (an empty B200
+    // leaves the 16 GiB standing; next to a simulation or other plans the plan shrinks instead of
+    // failing).  configure() halves the batch further if an allocation fails all the same.
+    size_t list_budget = size_t(16) << 30;
+    if (p->batch_auto) {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) list_budget = std::min(list_budget, free_b / 4);
+        else cudaGetLastError();
+    }
     const size_t frame_bytes = (size_t)p->n * p->max_nb * (sizeof(float4) + sizeof(uint32_t));
-    const int64_t mem_frames = std::max<int64_t>(1, (int64_t)((size_t(16) << 30) / frame_bytes));
+    const int64_t mem_frames = std::max<int64_t>(1, (int64_t)(list_budget / frame_bytes));
     if (p->batch_frames > mem_frames) p->batch_frames = (int32_t)mem_frames;
 
     ts->tri_warps = tiled_warps(p, ts->slab_bins_max);

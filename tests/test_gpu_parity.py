@@ -317,3 +317,35 @@ def test_normalize_merged_counts(oracle_lib, g3):
     assert np.array_equal((ca + cb).cpu().numpy().view(np.uint64), Ho)
     nz = Go != 0
     assert np.allclose(g.cpu().numpy()[nz], Go[nz], rtol=G3_RTOL, atol=0)
+
+
+def test_batch_shrinks_when_device_memory_is_short(g3):
+    """Config-4 shape with most of the GPU's memory taken by somebody else (an MD engine, other
+    plans): the automatic batch is sized from the free memory, an explicit batch that does not
+    fit is halved until it does, and the counts are those of the roomy plan."""
+    import torch
+    w = WORKLOADS[4]
+    _, pos = frames(w, 3)
+    d = torch.from_numpy(pos).cuda()
+
+    def run(**opts):
+        with g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, kernel=2, **opts) as plan:
+            plan.accumulate_frames(d)
+            c, _, st = plan.finalize(want_g3=False)
+            return c.clone(), st, plan.info(g3.G3_INFO_BATCH_FRAMES)
+
+    c0, st0, b0 = run()
+    assert b0 >= 64                                             # an empty B200: ~2^22 centres per batch
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    hog = torch.empty(free - (6 << 30), dtype=torch.uint8, device="cuda")     # leave 6 GiB
+    try:
+        c1, st1, b1 = run()                                     # lists <= a quarter of what is free
+        assert 1 <= b1 <= 12 and st1 == st0 and torch.equal(c1, c0)
+        c2, st2, b2 = run(batch_frames=64)                      # 64 frames of lists need 9.4 GB
+        assert 1 <= b2 <= 32 and st2 == st0 and torch.equal(c2, c0)
+    finally:
+        del hog
+        torch.cuda.empty_cache()
+    assert run()[2] == b0
