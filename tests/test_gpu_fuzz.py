@@ -25,7 +25,7 @@ def g3():
 def test_random_shapes(oracle_lib, g3, seed):
     import torch
     rng = np.random.default_rng(seed)
-    compared = checked_by_oracle = 0
+    compared = checked_by_oracle = tiled_compared = 0
     for _ in range(40):
         n = int(rng.integers(3, 6000))
         box = float(rng.uniform(1.0, 20.0))
@@ -47,7 +47,7 @@ def test_random_shapes(oracle_lib, g3, seed):
         pos = grid_to_pos(ms, box)
         d = torch.from_numpy(pos).cuda()
         wide = bool(rng.integers(0, 2))
-        res = {}
+        res, ran = {}, {}
         for kernel in (1, 2):
             try:
                 with g3.Plan(n, box, r_max, n_r, n_t, kernel=kernel, g2_wide=wide,
@@ -55,6 +55,7 @@ def test_random_shapes(oracle_lib, g3, seed):
                     plan.accumulate_frames(d)
                     c, _, st = plan.finalize(want_g3=False)
                     c2, _ = plan.finalize_g2()
+                    ran[kernel] = plan.info(g3.G3_INFO_KERNEL)   # kernel = 2 is a request: the plan may still choose 1
                     res[kernel] = (c.cpu().numpy().view(np.uint64), st, c2.cpu().numpy().view(np.uint64))
             except g3.G3Error as e:
                 res[kernel] = e.code
@@ -65,6 +66,8 @@ def test_random_shapes(oracle_lib, g3, seed):
         case = (n, box, r_max, n_r, n_t, kind, F, wide)
         assert np.array_equal(a[0], b[0]) and a[1] == b[1] and np.array_equal(a[2], b[2]), case
         compared += 1
+        assert ran[1] == 1
+        tiled_compared += ran[2] == 2
         if n * mean_k * mean_k < 2e8:
             orc = oracle_lib.Oracle(n, box, r_max, n_r, n_t, mode="allpairs" if n < 1500 else "cells")
             orc.accumulate(pos)
@@ -76,4 +79,5 @@ def test_random_shapes(oracle_lib, g3, seed):
                 oracle_lib.g2_frame(ms[f], T, H2)
             assert np.array_equal(a[2], H2), case
             checked_by_oracle += 1
-    assert compared >= 10 and checked_by_oracle >= 5
+    # at least ten of the comparisons really were tiled path against generic kernel
+    assert compared >= 10 and checked_by_oracle >= 5 and tiled_compared >= 10, (compared, checked_by_oracle, tiled_compared)
