@@ -57,6 +57,30 @@ def ncu_lsu_busy(kernel: str):
 
 ALGO_INSTR_PER_DISPLACEMENT = 9       # MSD: 3 subtractions, 3 multiply-adds, one 128-bit accumulate
 ALGO_INSTR_PER_QTET_ATOM = 210        # q_tet: exact keys + top-4 insertion of ~6 list-head entries (150) + Eq. 1 in fp64 (60)
+# wide g2: per candidate pair the second pair search tests (3 coordinate differences, 3 multiply-adds,
+# 1 comparison with the cut-off) and, per pair that lands in [r_max, 2 r_max), 2 for the shell and 1 add
+ALGO_INSTR_PER_G2W_CANDIDATE = 7
+ALGO_INSTR_PER_G2W_HIT = 3
+
+
+def g2w_candidate_pairs(pos_frame: np.ndarray, box: float, ncell: int) -> int:
+    """Unordered candidate pairs the wide-g2 search of one frame has to test on an ncell^3 grid: a
+    particle against the later members of its own cell and against the 62 cells of the forward half
+    of the 5x5x5 stencil (every pair within 2 r_max once).  Counted from the cell
+    occupancies of the frame, on the host, outside every timed region."""
+    m = np.rint(pos_frame * (1048576.0 / box)).astype(np.int64) % 1048576
+    cid = (m * ncell) >> 20
+    occ = np.zeros((ncell, ncell, ncell), dtype=np.int64)
+    np.add.at(occ, (cid[:, 0], cid[:, 1], cid[:, 2]), 1)
+    total = int((occ * (occ - 1) // 2).sum())
+    for dx in range(-2, 3):
+        for dy in range(-2, 3):
+            for dz in range(-2, 3):
+                if (dx, dy, dz) > (0, 0, 0):
+                    total += int((occ * np.roll(occ, (-dx, -dy, -dz), axis=(0, 1, 2))).sum())
+    return total
+
+
 TRAFFIC_PROFILES = {"tiled_triplet_kernel": "r2_triplet_kernel.md", "neighbour_cell_kernel": "r2_neighbour_kernel.md"}
 
 
@@ -314,6 +338,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream()
 
+    free_before = torch.cuda.mem_get_info()[0]
     plan = g3.Plan(w.n, w.box, w.r_max, w.n_r, w.n_t, timing=True,
                    batch_frames=args.batch_frames or None, triplet_warps=args.triplet_warps or None)
 
@@ -357,7 +382,16 @@ def run_ours(args):
             dist.all_reduce(ms, op=dist.ReduceOp.MAX)
         return float(ms.item()) / steps, out, t0, t1
 
-    for _ in range(max(args.warmup, 3)):
+    # the first step configures the plan (buffers sized for one batch, tables, memsets): its wall
+    # time and the device memory the plan then holds are reported, outside the timed region
+    t_first = time.time()
+    step_device()
+    torch.cuda.synchronize()
+    plan_info = {"first_step_ms": (time.time() - t_first) * 1e3,
+                 "device_bytes": int(free_before - torch.cuda.mem_get_info()[0]),
+                 "note": "free device memory before g3_plan_create minus after the first step "
+                         "(neighbour lists of one batch dominate; include/g3.h G3_OPT_BATCH_FRAMES)"}
+    for _ in range(max(args.warmup, 3) - 1):
         step_device()
     plan.clear_timing()
     sampler = ClockSampler(local)
@@ -475,6 +509,19 @@ def run_ours(args):
             pairs = int(c2w.cpu().numpy().view(np.uint64)[w.n_r:].sum())
             g2w = {"shells": 2 * w.n_r, "extra_ms_per_step": extra, "outer_ordered_pairs_per_step": pairs,
                    "outer_pairs_per_s_extra": pairs / (extra * 1e-3)}
+            ncell = gplan.info(g3.G3_INFO_CELLS_PER_EDGE)
+            if ncell >= 5:                       # the half-stencil kernel serves this grid
+                cand = g2w_candidate_pairs(pos[0], w.box, ncell) * F          # frames of one trajectory are alike
+                instr = cand * ALGO_INSTR_PER_G2W_CANDIDATE + (pairs // 2) * ALGO_INSTR_PER_G2W_HIT
+                g2w["roofline"] = {"bound": "alu", "unit": "Tinstr/s", "peak": peak_tinstr,
+                                   "kernel": "g2_wide_cell_kernel",
+                                   "candidate_pairs_per_step": cand,
+                                   "algorithmic_instr_per_candidate": ALGO_INSTR_PER_G2W_CANDIDATE,
+                                   "algorithmic_instr_per_hit": ALGO_INSTR_PER_G2W_HIT,
+                                   "achieved": instr / (extra * 1e-3) / 1e12,
+                                   "frac": instr / (extra * 1e-3) / 1e12 / peak_tinstr,
+                                   "note": "candidates counted from the cell occupancies of frame 0 x frames; "
+                                           "time = the extra device time of a step with G3_OPT_G2_WIDE"}
     except Exception as e:  # the g3 numbers above stay valid
         g2w = {"error": str(e)}
     # MSD over all time origins at the same shape (unwrapped random walk,
@@ -491,9 +538,24 @@ def run_ours(args):
         e1.record(stream)
         torch.cuda.synchronize()
         ms_msd = e0.elapsed_time(e1) / 3
+        # g3_msd_static: the same kernels with the scratch in libg3's built-in array (no allocation)
+        ms_msd_static = None
+        try:
+            s_out = torch.empty((F, 2), dtype=torch.int64, device="cuda")
+            m_out = torch.empty(F, dtype=torch.float64, device="cuda")
+            g3.msd_static(d_walk, w.box, sums=s_out, out=m_out)
+            e0.record(stream)
+            for _ in range(3):
+                g3.msd_static(d_walk, w.box, sums=s_out, out=m_out)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms_msd_static = e0.elapsed_time(e1) / 3
+        except g3.G3Error:                       # G3_ELIMIT: --frames beyond the built-in scratch
+            pass
         disp = w.n * F * (F + 1) // 2
         rate = disp / (ms_msd * 1e-3)
-        msd = {"ms": ms_msd, "displacements_per_s": rate, "frames": F, "lags": F,
+        msd = {"ms": ms_msd, "ms_no_alloc_entry": ms_msd_static,
+               "displacements_per_s": rate, "frames": F, "lags": F,
                "hbm_gbs_achieved": F * w.n * 24 / (ms_msd * 1e-3) / 1e9,
                "roofline": {"bound": "alu", "unit": "Tinstr/s", "peak": peak_tinstr,
                             "algorithmic_instr_per_displacement": ALGO_INSTR_PER_DISPLACEMENT,
@@ -532,6 +594,7 @@ def run_ours(args):
         "gpu_launches": launches * args.steps,
         "gpu_launches_per_step": launches,
         "roofline": roofline,
+        "plan": plan_info,
         "qtet": qtet,
         "g2_wide": g2w,
         "msd": msd,
