@@ -67,6 +67,25 @@ def test_strerror_and_argument_errors(lib):
     lib.g3_plan_destroy(None)
 
 
+def test_no_allocation_entry_point_limits_and_errors(lib):
+    """g3_msd_static (the MSD entry point for callers that cannot allocate device memory): the limit
+    the binding quotes is the header's, the scratch size follows from it, its own status code has a
+    description, and argument errors are reported before any CUDA call"""
+    import paper_1708_08619_b200 as g3
+    text = open(os.path.join(ROOT, "include", "g3.h")).read()
+    limit = int(re.search(r"#define G3_MSD_STATIC_MAX_PARTIALS (\d+)", text).group(1))
+    assert limit == g3.G3_MSD_STATIC_MAX_PARTIALS == 1 << 19
+    assert "#define G3_MSD_STATIC_SCRATCH_BYTES (256 + 16 * G3_MSD_STATIC_MAX_PARTIALS)" in text
+    assert (32768 // 32) * 500 <= limit                      # the config-4 shape with every lag fits
+    assert int(re.search(r"G3_ELIMIT = (\d+)", text).group(1)) == g3.G3_ELIMIT
+    assert "scratch" in g3.strerror(g3.G3_ELIMIT)
+    assert lib.g3_msd_static(None, 10, 10, 30, 1.0, 5, None, None, None) == g3.G3_EINVAL     # null positions
+    buf = ctypes.create_string_buffer(8)                     # never dereferenced: the arguments are refused first
+    assert lib.g3_msd_static(buf, 10, 10, 29, 1.0, 5, None, None, None) == g3.G3_EINVAL      # stride < 3 n
+    assert lib.g3_msd_static(buf, 10, 10, 30, 1.0, 10, None, None, None) == g3.G3_EINVAL     # max_lag > F - 1
+    assert lib.g3_msd_static(buf, 10, 10, 30, 0.0, 5, None, None, None) == g3.G3_EINVAL      # box
+
+
 def test_no_cpu_fallback_without_gpu(lib):
     """On a box without a CUDA device plan creation must fail loudly, never compute on the CPU."""
     import torch
