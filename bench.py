@@ -81,7 +81,7 @@ def g2w_candidate_pairs(pos_frame: np.ndarray, box: float, ncell: int) -> int:
     return total
 
 
-TRAFFIC_PROFILES = {"tiled_triplet_kernel": "r2_triplet_kernel.md", "neighbour_cell_kernel": "r2_neighbour_kernel.md"}
+TRAFFIC_PROFILES = {"tiled_triplet_kernel": "r3_triplet_kernel.md", "neighbour_cell_kernel": "r3_neighbour_kernel.md"}
 
 
 def ncu_traffic(kernel: str, frames_per_launch: int):
